@@ -1,0 +1,466 @@
+"""Pins for the CPU oracle (oracle/dnsref.c): each part is checked against something
+other than itself -- a library routine, a dense matrix built here from index
+arithmetic, a closed form, an exact amplification factor or an invariant.
+Numbering follows SURVEY.md section 8(c) (P1..P14).  CPU only.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import dnsref
+from paper_2204_02107_b200 import cases
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def rng(seed):
+    return np.random.default_rng(seed)
+
+
+def mk(shape, d=(1.0, 1.0, 1.0), nu=0.0, alpha_c=0.0, dt=1.0, **kw):
+    return dnsref.Oracle(shape, d, nu, alpha_c, dt, **kw)
+
+
+# ---------------------------------------------------------------- FFT (P0)
+@pytest.mark.parametrize("n", [1, 2, 4, 8, 16, 64, 12, 24])
+def test_fft1d_matches_definition_and_library(n):
+    r = rng(n)
+    re, im = r.standard_normal(n), r.standard_normal(n)
+    for sign in (-1, +1):
+        fr, fi = dnsref.fft1d(re, im, sign)
+        dr, di = dnsref.dft1d(re, im, sign)
+        lib = np.fft.fft(re + 1j * im) if sign < 0 else np.fft.ifft(re + 1j * im) * n
+        assert np.allclose(fr + 1j * fi, lib, rtol=0, atol=1e-12 * n)
+        assert np.allclose(dr + 1j * di, lib, rtol=0, atol=1e-12 * n)
+
+
+def test_fft1d_impulse_and_single_mode():
+    n = 32
+    re = np.zeros(n); im = np.zeros(n); re[3] = 1.0
+    fr, fi = dnsref.fft1d(re, im, -1)
+    k = np.arange(n)
+    assert np.allclose(fr, np.cos(2 * np.pi * 3 * k / n), atol=1e-14)
+    assert np.allclose(fi, -np.sin(2 * np.pi * 3 * k / n), atol=1e-14)  # forward sign is exp(-i...)
+
+
+def test_fft3_matches_library_nonsquare():
+    r = rng(7)
+    shape = (8, 4, 16)  # nz, ny, nx
+    a = r.standard_normal(shape) + 1j * r.standard_normal(shape)
+    fr, fi = dnsref.fft3(a.real, a.imag, -1)
+    assert np.allclose(fr + 1j * fi, np.fft.fftn(a), atol=1e-11)
+    br, bi = dnsref.fft3(fr, fi, +1)
+    assert np.allclose((br + 1j * bi) / a.size, a, atol=1e-13)
+
+
+# ---------------------------------------------------------------- dense operator (P1, P2)
+def _d1(n, h):
+    """Central first-difference circulant matrix, built from index arithmetic."""
+    D = np.zeros((n, n))
+    for i in range(n):
+        D[i, (i + 1) % n] += 1.0 / (2 * h)
+        D[i, (i - 1) % n] -= 1.0 / (2 * h)
+    return D
+
+
+def _dense_ops(shape, d):
+    nz, ny, nx = shape
+    Ix, Iy, Iz = np.eye(nx), np.eye(ny), np.eye(nz)
+    Dx = np.kron(Iz, np.kron(Iy, _d1(nx, d[0])))
+    Dy = np.kron(Iz, np.kron(_d1(ny, d[1]), Ix))
+    Dz = np.kron(_d1(nz, d[2]), np.kron(Iy, Ix))
+    return Dx, Dy, Dz
+
+
+def test_P1_dense_operator_spectrum_and_null_space():
+    shape, d = (8, 8, 8), (0.5, 0.7, 1.1)
+    Dx, Dy, Dz = _dense_ops(shape, d)
+    L = Dx @ Dx + Dy @ Dy + Dz @ Dz
+    assert np.allclose(L, L.T, atol=1e-14)
+    ev = np.sort(np.linalg.eigvalsh(L))
+    o = mk(shape, d)
+    lam = np.sort([o.eig(kx, ky, kz) for kz in range(8) for ky in range(8) for kx in range(8)])
+    assert np.allclose(ev, lam, atol=1e-12)
+    assert int(np.sum(np.abs(ev) < 1e-10)) == 8
+
+
+def test_P2_bruteforce_dense_poisson():
+    shape, d = (8, 8, 8), (0.5, 0.7, 1.1)
+    Dx, Dy, Dz = _dense_ops(shape, d)
+    L = Dx @ Dx + Dy @ Dy + Dz @ Dz
+    w, V = np.linalg.eigh(L)
+    Nn = V[:, np.abs(w) < 1e-10]          # orthonormal null-space basis (8 vectors)
+    assert Nn.shape[1] == 8
+    r = rng(11).standard_normal(512)
+    r_perp = r - Nn @ (Nn.T @ r)
+    p_dense = np.linalg.solve(L + Nn @ Nn.T, r_perp)   # Gaussian elimination, unique solution _|_ null
+    o = mk(shape, d)
+    p = o.poisson(r.reshape(shape)).ravel()            # the oracle zeroes the null modes of r itself
+    assert np.abs(p - p_dense).max() <= 1e-12 * np.abs(p_dense).max()
+    assert np.abs(Nn.T @ p).max() < 1e-13              # result carries no null-space component
+
+
+def test_P3_manufactured_single_modes():
+    shape, d = (16, 8, 32), (0.3, 0.45, 0.2)
+    nz, ny, nx = shape
+    o = mk(shape, d)
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    for (kx, ky, kz, ph) in [(1, 0, 0, 0.3), (0, 1, 0, 0.1), (0, 0, 1, 1.0), (3, 2, 5, 0.7), (8, 2, 4, 0.2),
+                             (15, 3, 7, 0.5), (31, 7, 15, 0.4), (16, 1, 0, 0.9)]:
+        p = np.cos(2 * np.pi * kx * i / nx + ph) * np.cos(2 * np.pi * ky * j / ny + 2 * ph) * \
+            np.cos(2 * np.pi * kz * k / nz - ph)
+        lam = -(math.sin(2 * math.pi * kx / nx) ** 2 / d[0] ** 2 + math.sin(2 * math.pi * ky / ny) ** 2 / d[1] ** 2 +
+                math.sin(2 * math.pi * kz / nz) ** 2 / d[2] ** 2)
+        assert abs(o.eig(kx, ky, kz) - lam) < 1e-13 * abs(lam)
+        got = o.poisson(lam * p)
+        assert np.abs(got - p).max() < 1e-13, (kx, ky, kz)
+
+
+def test_P4_projection_gives_roundoff_divergence():
+    shape, d = (24, 16, 32), (0.11, 0.17, 0.13)
+    r = rng(4)
+    us, vs, ws = (r.standard_normal(shape) for _ in range(3))
+    o = mk(shape, d)
+    dv = o.div(us, vs, ws)
+    # independent check of the divergence itself (np.roll form of the central difference)
+    ref = (np.roll(us, -1, 2) - np.roll(us, 1, 2)) / (2 * d[0]) + (np.roll(vs, -1, 1) - np.roll(vs, 1, 1)) / (2 * d[1]) \
+        + (np.roll(ws, -1, 0) - np.roll(ws, 1, 0)) / (2 * d[2])
+    assert np.abs(dv - ref).max() < 1e-12
+    p = o.poisson(dv)
+    u, v, w = o.project(us, vs, ws, p)
+    assert np.abs(o.div(u, v, w)).max() <= 1e-12 * np.abs(dv).max()
+    # gradient sign/axis: for p = sin(2 pi i/nx) only u changes, by -cos()*sin(2pi/nx)/dx
+    nz, ny, nx = shape
+    i = np.arange(nx)
+    p1 = np.broadcast_to(np.sin(2 * np.pi * i / nx), shape).copy()
+    u1, v1, w1 = o.project(us, vs, ws, p1)
+    assert np.array_equal(v1, vs) and np.array_equal(w1, ws)
+    assert np.allclose(us - u1, np.broadcast_to(np.cos(2 * np.pi * i / nx) * math.sin(2 * math.pi / nx) / d[0], shape),
+                       atol=1e-13)
+
+
+# ---------------------------------------------------------------- convection identities (P5, P6)
+def _solenoidal(shape, d, seed):
+    """Discretely solenoidal random field built here with numpy FFTs (independent of the oracle)."""
+    r = rng(seed)
+    nz, ny, nx = shape
+    f = [np.fft.fftn(r.standard_normal(shape)) for _ in range(3)]
+    mx = np.sin(2 * np.pi * np.fft.fftfreq(nx))[None, None, :] / d[0]
+    my = np.sin(2 * np.pi * np.fft.fftfreq(ny))[None, :, None] / d[1]
+    mz = np.sin(2 * np.pi * np.fft.fftfreq(nz))[:, None, None] / d[2]
+    m2 = mx * mx + my * my + mz * mz
+    ok = m2 > 1e-14
+    dot = np.where(ok, (mx * f[0] + my * f[1] + mz * f[2]) / np.where(ok, m2, 1.0), 0.0)
+    return [np.fft.ifftn(f[0] - dot * mx).real, np.fft.ifftn(f[1] - dot * my).real, np.fft.ifftn(f[2] - dot * mz).real]
+
+
+def test_P5_skew_symmetric_energy_identities():
+    shape, d = (12, 16, 20), (0.1, 0.13, 0.09)
+    r = rng(5)
+    u, v, w, c = (r.standard_normal(shape) for _ in range(4))
+    o = mk(shape, d, nu=0.0, alpha_c=0.0)
+    Fu, Fv, Fw, Fc = o.rhs(u, v, w, c)
+    scale = np.abs(u * Fu).sum() + np.abs(v * Fv).sum() + np.abs(w * Fw).sum()
+    assert abs((u * Fu + v * Fv + w * Fw).sum()) < 1e-13 * scale       # kinetic energy conserved for ANY u
+    assert abs((c * Fc).sum()) < 1e-13 * np.abs(c * Fc).sum()          # scalar variance conserved
+    assert abs(Fu.sum()) > 1e-3 * np.abs(Fu).sum() * 1e-3             # momentum NOT conserved if div u != 0
+
+
+def test_P6_momentum_conserved_for_solenoidal_field():
+    shape, d = (12, 16, 20), (0.1, 0.13, 0.09)
+    u, v, w = _solenoidal(shape, d, 6)
+    c = rng(66).standard_normal(shape)
+    o = mk(shape, d, nu=0.3, alpha_c=0.2)
+    assert np.abs(o.div(u, v, w)).max() < 1e-11
+    F = o.rhs(u, v, w, c)
+    for f in F:
+        assert abs(f.sum()) < 1e-11 * np.abs(f).sum()
+
+
+def test_rhs_constant_advection_of_linear_product():
+    """Sign and axis pin of each convective term: u = (U,V,W) constant, c = one cosine per axis.
+    F_c = -(U d_x c + V d_y c + W d_z c) with the central-difference symbol sin(theta)/D."""
+    shape, d = (8, 16, 32), (0.2, 0.3, 0.5)
+    nz, ny, nx = shape
+    U, V, W = 0.7, -0.4, 1.3
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    o = mk(shape, d)
+    one = np.ones(shape)
+    for ax, (n, idx, vel, h) in enumerate([(nx, i, U, d[0]), (ny, j, V, d[1]), (nz, k, W, d[2])]):
+        th = 2 * np.pi * 3 / n
+        c = np.sin(th * idx)
+        Fc = o.rhs(U * one, V * one, W * one, c)[3]
+        assert np.allclose(Fc, -vel * np.cos(th * idx) * math.sin(th) / h, atol=1e-13), ax
+
+
+# ---------------------------------------------------------------- exact linear solutions (P7, P8)
+def _G(z):
+    return 1 + z + z ** 2 / 2 + z ** 3 / 6 + z ** 4 / 24
+
+
+def test_P7_shear_flow_exact_rk4_amplification():
+    shape, d = (16, 8, 4), (0.4, 0.25, 0.2)
+    nz, ny, nx = shape
+    nu, ac, dt = 0.05, 0.03, 0.11
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    ty, tz = 2 * np.pi * 2 / ny, 2 * np.pi * 3 / nz
+    mode = np.cos(ty * j + 0.3) * np.cos(tz * k - 0.2)
+    zero = np.zeros(shape)
+    o = mk(shape, d, nu=nu, alpha_c=ac, dt=dt)
+    o.set_fields(1.7 * mode, zero, zero, -0.6 * mode)
+    nsteps = 3
+    o.step(nsteps)
+    f = o.fields()
+    sym = (2 * math.cos(ty) - 2) / d[1] ** 2 + (2 * math.cos(tz) - 2) / d[2] ** 2
+    assert np.abs(f["u"] - 1.7 * mode * _G(nu * dt * sym) ** nsteps).max() < 1e-14
+    assert np.abs(f["c"] + 0.6 * mode * _G(ac * dt * sym) ** nsteps).max() < 1e-14
+    assert np.abs(f["v"]).max() == 0 and np.abs(f["w"]).max() == 0 and np.abs(f["p"]).max() < 1e-15
+
+
+def test_P8_uniform_advection_exact_rk4_amplification():
+    shape, d = (8, 16, 32), (0.2, 0.3, 0.5)
+    nz, ny, nx = shape
+    U, V, W = 0.7, -0.4, 1.3
+    ac, dt = 0.02, 0.05
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    tx, ty, tz = 2 * np.pi * 3 / nx, 2 * np.pi * 1 / ny, 2 * np.pi * 2 / nz
+    phase = tx * i + ty * j + tz * k
+    one = np.ones(shape)
+    o = mk(shape, d, nu=0.01, alpha_c=ac, dt=dt)
+    o.set_fields(U * one, V * one, W * one, np.cos(phase))
+    o.step(2)
+    f = o.fields()
+    z = dt * (-1j * (U * math.sin(tx) / d[0] + V * math.sin(ty) / d[1] + W * math.sin(tz) / d[2])
+              + ac * ((2 * math.cos(tx) - 2) / d[0] ** 2 + (2 * math.cos(ty) - 2) / d[1] ** 2 +
+                      (2 * math.cos(tz) - 2) / d[2] ** 2))
+    expect = (np.exp(1j * phase) * _G(z) ** 2).real
+    assert np.abs(f["c"] - expect).max() < 1e-14
+    assert np.abs(f["u"] - U).max() < 1e-14 and np.abs(f["v"] - V).max() < 1e-14 and np.abs(f["w"] - W).max() < 1e-14
+
+
+# ---------------------------------------------------------------- paper's channel case (P9)
+def test_P9_poiseuille_fixed_point_with_mask_and_body_force():
+    """U(y) = (-b_x/2nu) y^2 + (b_x D/2nu) y is recovered in the masked channel.
+    Discretely it is an exact fixed point (the 3-point Laplacian is exact on a parabola)."""
+    rows = [l.split() for l in open(os.path.join(GOLD, "poiseuille.txt")) if not l.startswith("#")]
+    U = np.array([float(r[1]) for r in rows])
+    bx, nu, ny, dy, wall = 1.0e-3, 0.05, 32, 0.25, 2
+    shape = (4, ny, 8)
+    mask = np.ones(shape, dtype=np.uint8)
+    mask[:, :wall, :] = 0
+    mask[:, ny - wall:, :] = 0
+    u0 = np.broadcast_to(U[None, :, None], shape).copy()
+    zero = np.zeros(shape)
+    o = mk(shape, (0.3, dy, 0.4), nu=nu, alpha_c=nu, dt=0.2, mask=mask, body=(bx, 0.0, 0.0), n_piter=4)
+    o.set_fields(u0, zero, zero, mask.astype(float))
+    o.step(5)
+    f = o.fields()
+    assert np.abs(f["u"] - u0).max() < 1e-13 * U.max()
+    assert np.abs(f["v"]).max() < 1e-15 and np.abs(f["w"]).max() < 1e-15 and np.abs(f["p"]).max() < 1e-15
+    assert np.abs(f["c"] - mask).max() < 1e-14          # dc/dn = 0 at the walls keeps c = 1 in the fluid
+    # bulk velocity of the paper's closed form, continuous: b_x D^2 / (12 nu); the sampled mean is within O(dy^2)
+    D = (ny - wall - (wall - 1)) * dy
+    assert abs(U[wall - 1:ny - wall + 1].sum() * dy / D - bx * D * D / (12 * nu)) < 2e-3 * bx * D * D / (12 * nu)
+
+
+# ---------------------------------------------------------------- nonlinear closed forms (P10-P12)
+def _tgv2d(n, nu, dt, steps, flags=0):
+    h = 2 * math.pi / n
+    x = np.arange(n) * h
+    X, Y = np.meshgrid(x, x, indexing="xy")   # arrays [j, i]
+    u2, v2 = np.sin(X) * np.cos(Y), -np.cos(X) * np.sin(Y)
+    shape = (4, n, n)
+    u = np.broadcast_to(u2, shape).copy()
+    v = np.broadcast_to(v2, shape).copy()
+    o = mk(shape, (h, h, h), nu=nu, alpha_c=nu, dt=dt, flags=flags)
+    o.set_fields(u, v, np.zeros(shape), np.zeros(shape))
+    o.step(steps)
+    f = o.fields()
+    lam2 = 2 * (2 * math.cos(h) - 2) / h ** 2
+    return f, u, v, lam2
+
+
+def test_P11_taylor_green_2d_first_order_in_dt():
+    """2-D Taylor-Green is an exact NS solution; with one projection per step the scheme
+    is first order in dt: the error halves with dt (ratio 2 +- 0.1)."""
+    n, nu, T = 32, 0.01, 0.3 * (2 * math.pi / 32) * 8
+    errs = []
+    for steps in (8, 16, 32):
+        f, u, v, lam2 = _tgv2d(n, nu, T / steps, steps)
+        errs.append(np.abs(f["u"] - u * math.exp(nu * lam2 * T)).max())
+    assert 1.9 < errs[0] / errs[1] < 2.1 and 1.9 < errs[1] / errs[2] < 2.1
+    assert errs[0] < 5e-2
+
+
+def test_P11b_per_stage_projection_is_rk4_exact():
+    """NEXT-2 variant (flags bit1): projecting every stage makes 2-D Taylor-Green decay by RK4's G(z)."""
+    n, nu = 32, 0.01
+    dt = 0.3 * 2 * math.pi / n
+    f, u, v, lam2 = _tgv2d(n, nu, dt, 4, flags=2)
+    g = _G(nu * lam2 * dt) ** 4
+    assert np.abs(f["u"] - u * g).max() < 1e-13 and np.abs(f["v"] - v * g).max() < 1e-13
+
+
+def test_P10_linear_limit_of_full_step():
+    case = cases.taylor_green(16)
+    eps = 1e-6
+    o = mk(case["shape"], case["d"], nu=case["nu"], alpha_c=case["nu"], dt=case["dt"])
+    o.set_fields(eps * case["u"], eps * case["v"], eps * case["w"], case["c"])
+    o.step(4)
+    h = case["d"][0]
+    lam3 = 3 * (2 * math.cos(h) - 2) / h ** 2
+    g = _G(case["nu"] * lam3 * case["dt"]) ** 4
+    f = o.fields()
+    assert np.abs(f["u"] - eps * case["u"] * g).max() < 1e-5 * eps
+
+
+def test_P12_config1_taylor_green_energy_decay():
+    gold = np.array([[float(x) for x in l.split()] for l in open(os.path.join(GOLD, "tgv32_energy.txt"))
+                     if not l.startswith("#")])
+    case = cases.config(1)
+    o = mk(case["shape"], case["d"], nu=case["nu"], alpha_c=case["alpha_c"], dt=case["dt"], n_piter=1)
+    o.set_fields(case["u"], case["v"], case["w"], case["c"])
+    assert np.abs(o.div(case["u"], case["v"], case["w"])).max() < 1e-14   # initial field discretely solenoidal
+    E0 = sum((case[k] ** 2).sum() for k in "uvw")
+    done = 0
+    for step, e_proto, e_lin in gold:
+        o.step(int(step) - done)
+        done = int(step)
+        f = o.fields()
+        E = sum((f[k] ** 2).sum() for k in "uvw") / E0
+        assert abs(E - e_proto) < 5e-8, (step, E)        # the digits SURVEY.md prints
+        assert abs(E / e_lin - 1) < 0.02                  # "analytic viscous decay", 2 % (splitting + transfer)
+        assert np.abs(o.div(f["u"], f["v"], f["w"])).max() < 1e-13
+    h = case["d"][0]
+    lam3 = 3 * (2 * math.cos(h) - 2) / h ** 2
+    assert abs(math.exp(2 * case["nu"] * lam3 * 10 * case["dt"]) - gold[-1, 2]) < 1e-5
+
+
+# ---------------------------------------------------------------- mask and eq. 9 (P13)
+def _masked_lap_dense_free(p, beta, d):
+    """sum_a delta_a[ beta delta_a p ] (eq. 7's operator) written with np.roll."""
+    out = np.zeros_like(p)
+    for ax, h in ((2, d[0]), (1, d[1]), (0, d[2])):
+        g = beta * (np.roll(p, -1, ax) - np.roll(p, 1, ax)) / (2 * h)
+        out += (np.roll(g, -1, ax) - np.roll(g, 1, ax)) / (2 * h)
+    return out
+
+
+def test_eq9_fixed_point_is_the_masked_operator():
+    """If p satisfies eq. 7, sum_a delta_a[beta delta_a p] = d, then eq. 9's right-hand side equals
+    sum_a delta_a delta_a p and one solve returns p (up to its null-space part)."""
+    case = cases.duct_room(32, 16, 16)
+    shape, d, beta = case["shape"], case["d"], case["mask"].astype(float)
+    o = mk(shape, d, mask=case["mask"])
+    p = rng(9).standard_normal(shape)
+    p = o.poisson(_masked_lap_dense_free(p, np.ones(shape), d))     # strip the null-space component
+    dd = _masked_lap_dense_free(p, beta, d)
+    r = o.poisson_rhs(dd, p)
+    assert np.abs(r - _masked_lap_dense_free(p, np.ones(shape), d)).max() < 1e-10 * np.abs(r).max()
+    assert np.abs(o.poisson(r) - p).max() < 1e-11 * np.abs(p).max()
+    # with beta == 1 the bracket vanishes identically
+    o1 = mk(shape, d)
+    assert np.array_equal(o1.poisson_rhs(dd, p), dd)
+
+
+def test_P13_masked_step_invariants():
+    case = cases.duct_room(32, 16, 16, steps=5)
+    beta = case["mask"].astype(float)
+
+    def run(n_piter, steps, cold=False):
+        o = mk(case["shape"], case["d"], nu=case["nu"], alpha_c=case["alpha_c"], dt=case["dt"], mask=case["mask"],
+               sources=case["sources"], n_piter=n_piter)
+        o.set_fields(case["u"], case["v"], case["w"], case["c"])
+        o.step(steps)
+        return o, o.fields()
+
+    resid = []
+    for P in (1, 2, 4, 8, 40):
+        o, f = run(P, 1)
+        solid = case["mask"] == 0
+        for k in "uvwc":
+            assert np.all(f[k][solid] == 0.0) and not np.any(np.signbit(f[k][solid]))   # bit-exact +0.0
+        resid.append(np.abs(o.div(f["u"], f["v"], f["w"]) * beta).max())
+    assert all(resid[i + 1] <= resid[i] * (1 + 1e-12) for i in range(len(resid) - 1)), resid
+    assert resid[-1] < 0.5 * resid[0]
+    o, f = run(4, 5)
+    assert all(np.isfinite(f[k]).all() for k in "uvwcp")
+    # the source drives the duct towards u_set
+    s = case["sources"][0]
+    assert f["u"][s["lo"][2] + 1, s["lo"][1] + 1, 0] > 0.5 * s["u_set"][0]
+
+
+def test_source_table_eq5():
+    """eq. 5: S = 1 at the centre, 1/2 at |x-xc| = W/2, -> 0 far away, symmetric,
+    periodic; binary box for B <= 0."""
+    n, d = 64, 0.25
+    t = dnsref.source_table(n, d, lo=20, size=9, B=4.0)       # centre at cell 24, W/2 = 4.5 cells
+    assert t[24] == 1.0
+    assert np.allclose(t[24 - 10:24], t[25:24 + 11][::-1])
+    x = abs(np.arange(n) - 24.0) * d
+    W2 = 4.5 * d
+    with np.errstate(divide="ignore"):
+        ref = 0.5 * (1 - np.tanh(4.0 * (x / W2 - W2 / x)))
+    assert np.allclose(t, ref, atol=1e-15)
+    assert t[60] < 1e-12 and np.all((t >= 0) & (t <= 1))
+    half = dnsref.source_table(n, d, lo=20, size=8, B=4.0)     # W/2 = 4 cells: cell 23.5 +- 4 not on grid
+    assert abs(dnsref.source_table(64, 1.0, 10, 4, 3.0)[13] - 0.5 * (1 - math.tanh(3.0 * (1.5 / 2 - 2 / 1.5)))) < 1e-15
+    b = dnsref.source_table(16, 1.0, lo=14, size=4, B=0.0)
+    assert list(np.nonzero(b)[0]) == [0, 1, 14, 15]
+    w = dnsref.source_table(16, 1.0, lo=14, size=5, B=2.0)     # wraps across the seam: centre at cell 0
+    assert w[0] == 1.0 and np.allclose(w[1:8], w[15:8:-1])
+    assert half.max() <= 1.0
+
+
+# ---------------------------------------------------------------- symmetries (P14)
+def _run_case(case, steps, n_piter=None):
+    o = mk(case["shape"], case["d"], nu=case["nu"], alpha_c=case["alpha_c"], dt=case["dt"], mask=case["mask"],
+           sources=case["sources"], body=case["body"], n_piter=n_piter or case["n_piter"])
+    o.set_fields(case["u"], case["v"], case["w"], case["c"])
+    o.step(steps)
+    return o.fields()
+
+
+def test_P14_shift_symmetry():
+    case = cases.duct_room(32, 16, 16)
+    f0 = _run_case(case, 2)
+    sh = (3, 5, 7)  # z, y, x
+    c2 = dict(case)
+    for k in "uvwc":
+        c2[k] = np.roll(case[k], sh, (0, 1, 2))
+    c2["mask"] = np.roll(case["mask"], sh, (0, 1, 2))
+    nz, ny, nx = case["shape"]
+    c2["sources"] = [dict(s, lo=((s["lo"][0] + sh[2]) % nx, (s["lo"][1] + sh[1]) % ny, (s["lo"][2] + sh[0]) % nz))
+                     for s in case["sources"]]
+    f1 = _run_case(c2, 2)
+    for k in "uvwcp":
+        ref = np.roll(f0[k], sh, (0, 1, 2))
+        assert np.abs(f1[k] - ref).max() <= 1e-12 * max(np.abs(ref).max(), 1e-300), k
+
+
+def test_P14_axis_permutation_symmetry():
+    """Swap x and z everywhere (fields, components, spacings, mask, sources): outputs swap too."""
+    case = cases.duct_room(32, 16, 8)
+    case["d"] = (0.05, 0.07, 0.06)
+    f0 = _run_case(case, 2)
+    T = lambda a: np.ascontiguousarray(a.transpose(2, 1, 0))
+    c2 = dict(case)
+    c2["shape"] = case["shape"][::-1]
+    c2["d"] = case["d"][::-1]
+    c2["u"], c2["v"], c2["w"], c2["c"] = T(case["w"]), T(case["v"]), T(case["u"]), T(case["c"])
+    c2["mask"] = T(case["mask"])
+    c2["sources"] = [dict(s, lo=s["lo"][::-1], size=s["size"][::-1], u_set=s["u_set"][::-1]) for s in case["sources"]]
+    f1 = _run_case(c2, 2)
+    for a, b in (("u", "w"), ("v", "v"), ("w", "u"), ("c", "c"), ("p", "p")):
+        ref = T(f0[b])
+        assert np.abs(f1[a] - ref).max() <= 1e-12 * max(np.abs(ref).max(), 1e-300), a
+
+
+def test_momentum_drift_bound_full_step():
+    """P6, full step: stages are unprojected, so mean velocity drifts slightly -- bound, not equality."""
+    case = cases.periodic_turbulence(32, steps=1)
+    f = _run_case(case, 1)
+    for k in "uvw":
+        assert 0 < abs(f[k].mean() - case[k].mean()) < 1e-4      # 32^3, k0 = 4: ~2e-5 u' per step
