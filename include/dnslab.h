@@ -1,0 +1,117 @@
+/*
+ * dnslab.h -- C ABI of libdnslab.so: the DNSLABIB incompressible Navier-Stokes time step
+ * (arxiv 2204.02107; citations are PAPER.md:<line>) on one NVIDIA B200 (sm_100a), fp64.
+ *
+ * The library owns no device memory: the caller hands it one device workspace and a CUDA
+ * stream (in this repo both come from PyTorch).  Every call is asynchronous on that stream
+ * unless stated otherwise.  All functions return 0 (DNSLAB_OK) or a negative error code;
+ * nothing throws across this boundary.  dnslab_strerror() gives text for a code.
+ *
+ * Grid and layout.  nx*ny*nz cells, all axes periodic, spacings dx,dy,dz.
+ * A field is nx*ny*nz doubles, x fastest: element (i,j,k) is at i + nx*(j + ny*k)
+ * (a contiguous torch/numpy array of shape (nz,ny,nx)).  nx,ny,nz must be powers of two with
+ * 8 <= nx <= 2048 and 8 <= ny,nz <= 1024 (the Poisson solve is a radix FFT).  The mask beta is one byte per cell,
+ * same layout, non-zero = fluid, 0 = solid.
+ *
+ * What one step computes (PAPER.md:43 and eqs. 1-4, 7-9; DESIGN.md lists every reading):
+ *   Qc = Q^n, Qs = Q^n                    Q = (u,v,w,c)
+ *   for s = 1..4 (classical RK4, a=(1/2,1/2,1), b=(1/6,1/3,1/3,1/6)):
+ *       F = beta ? RHS(Qs) : +0.0         eqs. 2-3: skew-symmetric central convection,
+ *                                         central diffusion (beta-weighted faces for c, eq. 4),
+ *                                         body force b, source relaxation S (phi_set - phi)/tau_f
+ *       Qc += b_s dt F ;  Qs = Q^n + a_s dt F   (s < 4)
+ *   d = sum_a delta_a Qc.u_a                                     (eq. 7 right-hand side)
+ *   repeat n_piter times (eq. 9; p starts from the previous step's p):
+ *       r = d + sum_a delta_a[(1-beta) delta_a p] ;  p = F^-1[ F[r] / lambda ]
+ *       lambda = -sum_a sin^2(2 pi k_a/N_a)/D_a^2 ; the 8 null modes (2 k_a = 0 mod N_a) := 0
+ *   u_a^{n+1} = beta ? Qc.u_a - delta_a p : +0.0 ;  c^{n+1} = Qc.c        (eq. 8)
+ * delta_a is the periodic central difference (f[+1]-f[-1])/(2 D_a).
+ */
+#ifndef DNSLAB_H
+#define DNSLAB_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DNSLAB_OK 0
+#define DNSLAB_EINVAL (-1) /* null pointer, bad dims/spacings/dt/nu/n_piter/tau_f, misaligned workspace */
+#define DNSLAB_ENOMEM (-2) /* workspace smaller than dnslab_workspace_bytes()                         */
+#define DNSLAB_ECUDA (-3)  /* a CUDA call or kernel launch failed (sticky error)                      */
+#define DNSLAB_EARCH (-4)  /* no device, or the current device is not compute capability 10.x         */
+
+#define DNSLAB_MAX_SOURCES 16
+
+typedef struct dnslab dnslab_t; /* opaque handle; host memory owned by the library */
+
+typedef struct {
+    int32_t nx, ny, nz;    /* grid, powers of two: nx in [8,2048], ny,nz in [8,1024]                 */
+    double dx, dy, dz;     /* spacings > 0                                                           */
+    double nu;             /* kinematic viscosity >= 0 (eq. 2)                                       */
+    double alpha_c;        /* scalar diffusivity >= 0 (eq. 3)                                        */
+    double dt;             /* fixed time step > 0                                                    */
+    double body[3];        /* body force b (eq. 2)                                      */
+    int32_t n_piter;       /* eq. 9 iterations >= 1; the paper hard-codes 4           */
+    uint32_t flags;        /* bit0 reserved (eq. 6 filter, not built); bit1: project every RK stage  */
+} dnslab_params_t;
+
+/* One inflow/outflow forcing region S(x,y,z) of eqs. 2-3. */
+typedef struct {
+    int32_t lo[3], size[3]; /* index box in x,y,z: cells lo..lo+size-1, wrapping modulo N            */
+    double B[3];            /* eq. 5 smoothness per axis; B <= 0: binary S = 1 inside the box.
+                               B > 0: S_a = (1 - tanh(B[r/(W/2) - (W/2)/r]))/2, r = |x - xc| by
+                               minimum image, xc = (lo + (size-1)/2) D, W = size D, S_a(xc) = 1      */
+    double u_set[3], c_set; /* target values                                                          */
+    double tau_f;           /* relaxation time > 0                                                    */
+    uint32_t comps;         /* bit0..3: force u, v, w, c                                              */
+} dnslab_source_t;
+
+/* Bytes of device workspace dnslab_create needs for these params; 0 if the params are invalid. */
+size_t dnslab_workspace_bytes(const dnslab_params_t *params);
+
+/*
+ * Create a solver.  mask: nx*ny*nz bytes (host or device pointer; NULL = all fluid), copied.
+ * src: nsrc (<= DNSLAB_MAX_SOURCES) host structs, copied.  workspace: DEVICE memory, caller-owned,
+ * at least dnslab_workspace_bytes() bytes, 256-byte aligned; it must outlive the handle.
+ * cuda_stream: a cudaStream_t (NULL = default stream); every later call runs on it.
+ * All fields start at 0 (p = 0 is the first warm start).  Synchronous.
+ */
+int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnslab_source_t *src, int32_t nsrc,
+                  void *workspace, void *cuda_stream, dnslab_t **out);
+
+/* Copy fields in (host or device pointers, nx*ny*nz doubles each).  u,v,w,c are stored as
+ * beta ? x : +0.0; p may be NULL (-> 0) and is not masked. */
+int dnslab_set_fields(dnslab_t *h, const double *u, const double *v, const double *w, const double *c,
+                      const double *p);
+
+/* Advance n >= 0 full time steps.  Asynchronous; no host synchronisation inside. */
+int dnslab_step(dnslab_t *h, int32_t n);
+
+/* One Poisson solve with the beta term off: p = F^-1[F[rhs]/lambda], null modes 0 (eq. 9 with
+ * beta = 1).  rhs and p are DEVICE pointers to nx*ny*nz doubles; they may alias.  Does not
+ * touch the solver's own pressure. */
+int dnslab_poisson(dnslab_t *h, const double *rhs, double *p);
+
+/* Borrowed DEVICE pointers to the current u,v,w,c,p (any out-pointer may be NULL).  No copy.
+ * Valid until the next dnslab_step / dnslab_set_fields / dnslab_destroy (buffers rotate). */
+int dnslab_fields(dnslab_t *h, const double **u, const double **v, const double **w, const double **c,
+                  const double **p);
+
+/* Copy the current fields out to host or device buffers (any may be NULL).  Asynchronous on the
+ * stream for device and pinned-host destinations; synchronise the stream before reading. */
+int dnslab_get_fields(dnslab_t *h, double *u, double *v, double *w, double *c, double *p);
+
+/* Number of kernels the library has launched on this handle since create (for bench accounting). */
+int64_t dnslab_launch_count(const dnslab_t *h);
+
+int dnslab_destroy(dnslab_t *h);
+
+const char *dnslab_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DNSLAB_H */

@@ -1,0 +1,203 @@
+"""Thin Python binding over the C ABI of libdnslab.so (include/dnslab.h).
+
+Argument marshalling only: every step of the hot path runs in the library's CUDA kernels.
+PyTorch provides the device workspace and the stream, nothing else.  There is no CPU
+fallback: if the library is missing or no sm_100 GPU is present the calls raise.
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdnslab.so")
+
+SYMBOLS = ["dnslab_workspace_bytes", "dnslab_create", "dnslab_set_fields", "dnslab_step", "dnslab_poisson",
+           "dnslab_fields", "dnslab_get_fields", "dnslab_launch_count", "dnslab_destroy", "dnslab_strerror"]
+
+
+class Params(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
+                ("nu", C.c_double), ("alpha_c", C.c_double), ("dt", C.c_double),
+                ("body", C.c_double * 3), ("n_piter", C.c_int32), ("flags", C.c_uint32)]
+
+
+class Source(C.Structure):
+    _fields_ = [("lo", C.c_int32 * 3), ("size", C.c_int32 * 3), ("B", C.c_double * 3),
+                ("u_set", C.c_double * 3), ("c_set", C.c_double), ("tau_f", C.c_double),
+                ("comps", C.c_uint32)]
+
+
+class DnslabError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """Load libdnslab.so (built in-tree by paper_2204_02107_b200/build.py).  Fails loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise DnslabError(f"{LIB_PATH} not built: run `python -m paper_2204_02107_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.dnslab_workspace_bytes.argtypes = [C.POINTER(Params)]
+        L.dnslab_workspace_bytes.restype = C.c_size_t
+        L.dnslab_create.argtypes = [C.POINTER(Params), C.c_void_p, C.POINTER(Source), C.c_int32, C.c_void_p,
+                                    C.c_void_p, C.POINTER(C.c_void_p)]
+        L.dnslab_set_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 5
+        L.dnslab_step.argtypes = [C.c_void_p, C.c_int32]
+        L.dnslab_poisson.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.dnslab_fields.argtypes = [C.c_void_p] + [C.POINTER(C.c_void_p)] * 5
+        L.dnslab_get_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 5
+        L.dnslab_launch_count.argtypes = [C.c_void_p]
+        L.dnslab_launch_count.restype = C.c_int64
+        L.dnslab_destroy.argtypes = [C.c_void_p]
+        L.dnslab_strerror.argtypes = [C.c_int]
+        L.dnslab_strerror.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise DnslabError(f"{what} failed: {lib().dnslab_strerror(rc).decode()} ({rc})")
+
+
+def make_params(shape, d, nu, alpha_c, dt, body=(0.0, 0.0, 0.0), n_piter=1, flags=0):
+    nz, ny, nx = (int(s) for s in shape)
+    P = Params()
+    P.nx, P.ny, P.nz = nx, ny, nz
+    P.dx, P.dy, P.dz = (float(x) for x in d)
+    P.nu, P.alpha_c, P.dt = float(nu), float(alpha_c), float(dt)
+    P.body[:] = [float(b) for b in body]
+    P.n_piter, P.flags = int(n_piter), int(flags)
+    return P
+
+
+def make_sources(sources):
+    arr = (Source * max(1, len(sources)))()
+    for s, d in zip(arr, sources):
+        s.lo[:] = [int(x) for x in d["lo"]]
+        s.size[:] = [int(x) for x in d["size"]]
+        s.B[:] = d.get("B", (0.0, 0.0, 0.0))
+        s.u_set[:] = d.get("u_set", (0.0, 0.0, 0.0))
+        s.c_set = d.get("c_set", 0.0)
+        s.tau_f = d["tau_f"]
+        s.comps = d.get("comps", 0xF)
+    return arr
+
+
+def workspace_bytes(params):
+    return int(lib().dnslab_workspace_bytes(C.byref(params)))
+
+
+def _addr(x):
+    """Address of a torch tensor (device or host), a numpy array, or None."""
+    if x is None:
+        return None
+    if hasattr(x, "data_ptr"):
+        assert x.is_contiguous()
+        return x.data_ptr()
+    assert x.flags["C_CONTIGUOUS"]
+    return x.ctypes.data
+
+
+class Solver:
+    """dnslab_create / set_fields / step / poisson / fields / get_fields / destroy.
+
+    Arrays are (nz, ny, nx), x fastest.  `mask` (uint8, 1 = fluid) and the inputs of set_fields /
+    outputs of get_fields may be host (numpy or torch CPU) or device (torch CUDA) buffers.
+    """
+
+    def __init__(self, shape, d, nu, alpha_c, dt, mask=None, sources=(), body=(0.0, 0.0, 0.0), n_piter=1, flags=0,
+                 device="cuda:0", stream=None):
+        import torch  # device memory and streams only
+        if not torch.cuda.is_available():
+            raise DnslabError("no CUDA device: the DNSLAB path has no CPU fallback")
+        self._torch = torch
+        self.shape = tuple(int(s) for s in shape)
+        self.device = torch.device(device)
+        self.params = make_params(self.shape, d, nu, alpha_c, dt, body, n_piter, flags)
+        nbytes = workspace_bytes(self.params)
+        if nbytes == 0:
+            raise DnslabError("invalid parameters (dnslab_workspace_bytes returned 0)")
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        self._ws_ptr = (base + 255) // 256 * 256
+        self._src = make_sources(list(sources))
+        self._h = C.c_void_p()
+        if mask is not None and hasattr(mask, "dtype") and not hasattr(mask, "data_ptr"):
+            import numpy as np
+            mask = np.ascontiguousarray(mask, dtype=np.uint8)
+        self._mask = mask
+        _check(lib().dnslab_create(C.byref(self.params), _addr(mask), self._src, len(sources), self._ws_ptr,
+                                   self.stream.cuda_stream, C.byref(self._h)), "dnslab_create")
+
+    # -- C ABI calls ---------------------------------------------------------------------
+    def set_fields(self, u, v, w, c, p=None):
+        self._keep = (u, v, w, c, p)  # keep host buffers alive until the async copies ran
+        _check(lib().dnslab_set_fields(self._h, _addr(u), _addr(v), _addr(w), _addr(c), _addr(p)), "dnslab_set_fields")
+
+    def step(self, n=1):
+        _check(lib().dnslab_step(self._h, int(n)), "dnslab_step")
+
+    def poisson(self, rhs, out=None):
+        torch = self._torch
+        assert rhs.is_cuda and rhs.dtype == torch.float64 and rhs.is_contiguous()
+        if out is None:
+            out = torch.empty_like(rhs)
+        _check(lib().dnslab_poisson(self._h, rhs.data_ptr(), out.data_ptr()), "dnslab_poisson")
+        return out
+
+    def field_ptrs(self):
+        ptrs = [C.c_void_p() for _ in range(5)]
+        _check(lib().dnslab_fields(self._h, *[C.byref(p) for p in ptrs]), "dnslab_fields")
+        return dict(zip("uvwcp", (p.value for p in ptrs)))
+
+    def get_fields(self, u=None, v=None, w=None, c=None, p=None):
+        _check(lib().dnslab_get_fields(self._h, _addr(u), _addr(v), _addr(w), _addr(c), _addr(p)), "dnslab_get_fields")
+
+    def launch_count(self):
+        return int(lib().dnslab_launch_count(self._h))
+
+    # -- conveniences (marshalling only) ---------------------------------------------------
+    def fields(self):
+        """Device copies of u,v,w,c,p as torch tensors."""
+        torch = self._torch
+        out = {k: torch.empty(self.shape, dtype=torch.float64, device=self.device) for k in "uvwcp"}
+        with torch.cuda.stream(self.stream):
+            self.get_fields(**out)
+        return out
+
+    def fields_numpy(self):
+        f = self.fields()
+        self.stream.synchronize()
+        return {k: t.cpu().numpy() for k, t in f.items()}
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.stream.synchronize()
+            lib().dnslab_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def solver_for_case(case, n_piter=None, flags=0, **kw):
+    """Solver for a dict from paper_2204_02107_b200.cases, fields loaded from its host arrays."""
+    s = Solver(case["shape"], case["d"], case["nu"], case["alpha_c"], case["dt"], mask=case["mask"],
+               sources=case["sources"], body=case["body"], n_piter=n_piter or case["n_piter"], flags=flags, **kw)
+    s.set_fields(case["u"], case["v"], case["w"], case["c"])
+    s.synchronize()
+    return s

@@ -1,0 +1,532 @@
+// dnslab.cu -- host side of libdnslab.so (C ABI in include/dnslab.h): workspace carving, table
+// set-up, launch sequence of one DNSLABIB time step.  No device allocation, no host sync in step.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/dnslab.h"
+#include "fft.cuh"
+#include "stencil.cuh"
+
+using dnsfft::c2;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+inline bool pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+bool valid_params(const dnslab_params_t *P)
+{
+    if (!P) return false;
+    if (!pow2(P->nx) || !pow2(P->ny) || !pow2(P->nz)) return false;
+    if (P->nx < 8 || P->nx > 2048 || P->ny < 8 || P->ny > 1024 || P->nz < 8 || P->nz > 1024) return false;
+    if (!(P->dx > 0) || !(P->dy > 0) || !(P->dz > 0) || !(P->dt > 0)) return false;
+    if (!(P->nu >= 0) || !(P->alpha_c >= 0) || P->n_piter < 1) return false;
+    if (P->flags & ~2u) return false;
+    return true;
+}
+
+struct Layout {
+    size_t field_bytes, off_fields, nfields, off_face, off_tw[3], off_eig, off_stab, total;
+};
+
+// 19 fields: Q(4) A(4) B(4) Qc(4) p d W (+1 scratch pressure with per-stage projection)
+Layout make_layout(const dnslab_params_t *P)
+{
+    Layout L;
+    const size_t n = (size_t)P->nx * P->ny * P->nz;
+    L.field_bytes = align_up(n * sizeof(double));
+    L.nfields = 19 + ((P->flags & 2u) ? 1 : 0);
+    size_t off = 0;
+    L.off_fields = off;
+    off += L.nfields * L.field_bytes;
+    L.off_face = off;
+    off += align_up(n);
+    const int len[3] = {P->nx / 2, P->ny, P->nz};
+    for (int a = 0; a < 3; ++a) {
+        L.off_tw[a] = off;
+        off += align_up((size_t)len[a] * sizeof(c2));
+    }
+    L.off_eig = off;
+    off += align_up((size_t)(P->nx / 2 + P->ny + P->nz) * sizeof(double));
+    L.off_stab = off;
+    off += align_up((size_t)DNSLAB_MAX_SOURCES * (P->nx + P->ny + P->nz) * sizeof(double));
+    L.total = off;
+    return L;
+}
+
+// eq. 5 one-dimensional factor; reading R10
+void source_profile(int n, double d, int lo, int size, double B, double *out)
+{
+    for (int i = 0; i < n; ++i) {
+        if (!(B > 0.0)) {
+            const int rel = (((i - lo) % n) + n) % n;
+            out[i] = rel < size ? 1.0 : 0.0;
+            continue;
+        }
+        const double len = n * d, centre = (lo + 0.5 * (size - 1)) * d, halfw = 0.5 * size * d;
+        double r = std::fmod(std::fabs(i * d - centre), len);
+        if (r > 0.5 * len) r = len - r;
+        out[i] = (r == 0.0) ? 1.0 : 0.5 * (1.0 - std::tanh(B * (r / halfw - halfw / r)));
+    }
+}
+
+} // namespace
+
+struct dnslab {
+    dnslab_params_t P;
+    size_t n;
+    cudaStream_t stream;
+    char *ws;
+    Layout L;
+    double *Q[4], *A[4], *Bf[4], *Qc[4], *p, *d, *W, *ps;
+    uint8_t *face; // null when the mask has no solid cell
+    c2 *tw[3];
+    double *eig[3];
+    double *stab;
+    int nsrc;
+    dnsst::SourceDev src[DNSLAB_MAX_SOURCES];
+    int64_t launches;
+    int zchunk;
+};
+
+namespace {
+
+#define CK(call)                                   \
+    do {                                           \
+        cudaError_t e_ = (call);                   \
+        if (e_ != cudaSuccess) return DNSLAB_ECUDA; \
+    } while (0)
+
+inline int check_launch(dnslab *h)
+{
+    h->launches++;
+    return cudaPeekAtLastError() == cudaSuccess ? DNSLAB_OK : DNSLAB_ECUDA;
+}
+
+dim3 tile_block(const dnslab *h)
+{
+    const int bx = h->P.nx < 32 ? h->P.nx : 32;
+    int by = 256 / bx;
+    if (by > h->P.ny) by = h->P.ny;
+    return dim3(bx, by, 1);
+}
+
+// ---- RK stage ---------------------------------------------------------------------------
+template <int STAGE> int launch_rk(dnslab *h, double *const *qs, double *const *qo)
+{
+    static const double ca[4] = {0.5, 0.5, 1.0, 0.0};
+    static const double cb[4] = {1.0 / 6.0, 1.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0};
+    dnsst::RKArgs a;
+    std::memset(&a, 0, sizeof(a));
+    for (int m = 0; m < 4; ++m) {
+        a.qs[m] = qs[m];
+        a.qn[m] = h->Q[m];
+        a.qc[m] = h->Qc[m];
+        a.qo[m] = qo ? qo[m] : nullptr;
+        a.qco[m] = h->Qc[m];
+    }
+    a.face = h->face;
+    a.nx = h->P.nx; a.ny = h->P.ny; a.nz = h->P.nz; a.zchunk = h->zchunk;
+    a.r2x = 1.0 / (2.0 * h->P.dx); a.r2y = 1.0 / (2.0 * h->P.dy); a.r2z = 1.0 / (2.0 * h->P.dz);
+    a.rxx = 1.0 / (h->P.dx * h->P.dx); a.ryy = 1.0 / (h->P.dy * h->P.dy); a.rzz = 1.0 / (h->P.dz * h->P.dz);
+    a.nu = h->P.nu; a.ac = h->P.alpha_c;
+    for (int m = 0; m < 3; ++m) a.body[m] = h->P.body[m];
+    a.ca = ca[STAGE - 1] * h->P.dt;
+    a.cb = cb[STAGE - 1] * h->P.dt;
+    a.nsrc = h->nsrc;
+    a.stab = h->stab;
+    for (int s = 0; s < h->nsrc; ++s) a.src[s] = h->src[s];
+    const dim3 blk = tile_block(h);
+    const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz / h->zchunk);
+    const bool masked = h->face != nullptr, sources = h->nsrc > 0;
+    if (masked && sources) dnsst::k_rk_stage<STAGE, true, true><<<grd, blk, 0, h->stream>>>(a);
+    else if (masked) dnsst::k_rk_stage<STAGE, true, false><<<grd, blk, 0, h->stream>>>(a);
+    else if (sources) dnsst::k_rk_stage<STAGE, false, true><<<grd, blk, 0, h->stream>>>(a);
+    else dnsst::k_rk_stage<STAGE, false, false><<<grd, blk, 0, h->stream>>>(a);
+    return check_launch(h);
+}
+
+// ---- FFT passes -------------------------------------------------------------------------
+template <int L> constexpr int col_xt() { return L >= 1024 ? 4 : (L >= 256 ? 8 : 16); }
+
+template <int L, int DIR, bool PRO> int launch_fft_x_L(dnslab *h, const c2 *in, c2 *out, const dnsfft::PoissonRhsArgs &ra)
+{
+    constexpr int E = dnsfft::ElemsPerThread<L>::value;
+    constexpr int T = L / E;
+    const size_t nlines = (size_t)h->P.ny * h->P.nz;
+    size_t nl = 256 / T;
+    if (nl > nlines) nl = nlines;
+    const size_t smem = nl * (L + L / 8) * sizeof(c2);
+    dnsfft::k_fft_x<L, DIR, PRO><<<(unsigned)(nlines / nl), (unsigned)(nl * T), smem, h->stream>>>(in, out, h->tw[0], (int)nl, ra);
+    return check_launch(h);
+}
+
+template <int DIR, bool PRO> int launch_fft_x(dnslab *h, const c2 *in, c2 *out, const dnsfft::PoissonRhsArgs &ra)
+{
+    switch (h->P.nx / 2) {
+    case 4: return launch_fft_x_L<4, DIR, PRO>(h, in, out, ra);
+    case 8: return launch_fft_x_L<8, DIR, PRO>(h, in, out, ra);
+    case 16: return launch_fft_x_L<16, DIR, PRO>(h, in, out, ra);
+    case 32: return launch_fft_x_L<32, DIR, PRO>(h, in, out, ra);
+    case 64: return launch_fft_x_L<64, DIR, PRO>(h, in, out, ra);
+    case 128: return launch_fft_x_L<128, DIR, PRO>(h, in, out, ra);
+    case 256: return launch_fft_x_L<256, DIR, PRO>(h, in, out, ra);
+    case 512: return launch_fft_x_L<512, DIR, PRO>(h, in, out, ra);
+    case 1024: return launch_fft_x_L<1024, DIR, PRO>(h, in, out, ra);
+    }
+    return DNSLAB_EINVAL;
+}
+
+template <typename K> int set_smem(K kernel, size_t smem)
+{
+    if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    return DNSLAB_OK;
+}
+
+// y pass: axis 1; z pass (unfused, used only by tests of the transform itself): axis 2
+template <int L, int XT, int DIR> int launch_fft_col_LX(dnslab *h, c2 *data, int axis)
+{
+    constexpr int T = L / dnsfft::ElemsPerThread<L>::value;
+    const int mx = h->P.nx / 2;
+    const size_t stride = axis == 1 ? (size_t)mx : (size_t)mx * h->P.ny;
+    const size_t other_stride = axis == 1 ? (size_t)mx * h->P.ny : (size_t)mx;
+    const int nother = axis == 1 ? h->P.nz : h->P.ny;
+    const size_t smem = (size_t)XT * L * sizeof(c2);
+    auto kern = dnsfft::k_fft_col<L, XT, DIR>;
+    if (int rc = set_smem(kern, smem)) return rc;
+    kern<<<(unsigned)((mx / XT) * nother), XT * T, smem, h->stream>>>(data, h->tw[axis], mx, stride, other_stride);
+    return check_launch(h);
+}
+
+template <int L, int DIR> int launch_fft_col_L(dnslab *h, c2 *data, int axis)
+{
+    constexpr int XT = col_xt<L>();
+    if (h->P.nx / 2 >= XT) return launch_fft_col_LX<L, XT, DIR>(h, data, axis);
+    return launch_fft_col_LX<L, 4, DIR>(h, data, axis);
+}
+
+template <int DIR> int launch_fft_col(dnslab *h, c2 *data, int axis)
+{
+    switch (axis == 1 ? h->P.ny : h->P.nz) {
+    case 8: return launch_fft_col_L<8, DIR>(h, data, axis);
+    case 16: return launch_fft_col_L<16, DIR>(h, data, axis);
+    case 32: return launch_fft_col_L<32, DIR>(h, data, axis);
+    case 64: return launch_fft_col_L<64, DIR>(h, data, axis);
+    case 128: return launch_fft_col_L<128, DIR>(h, data, axis);
+    case 256: return launch_fft_col_L<256, DIR>(h, data, axis);
+    case 512: return launch_fft_col_L<512, DIR>(h, data, axis);
+    case 1024: return launch_fft_col_L<1024, DIR>(h, data, axis);
+    }
+    return DNSLAB_EINVAL;
+}
+
+template <int L, int XT> int launch_fft_z_solve_LX(dnslab *h, c2 *data)
+{
+    constexpr int T = L / dnsfft::ElemsPerThread<L>::value;
+    const int mx = h->P.nx / 2;
+    const size_t smem = (size_t)XT * L * sizeof(c2);
+    auto kern = dnsfft::k_fft_z_solve<L, XT>;
+    if (int rc = set_smem(kern, smem)) return rc;
+    const double inv_n = 1.0 / (double)h->n;
+    kern<<<(unsigned)((mx / XT) * h->P.ny), XT * T, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], inv_n);
+    return check_launch(h);
+}
+
+template <int L> int launch_fft_z_solve_L(dnslab *h, c2 *data)
+{
+    constexpr int XT = col_xt<L>();
+    if (h->P.nx / 2 >= XT) return launch_fft_z_solve_LX<L, XT>(h, data);
+    return launch_fft_z_solve_LX<L, 4>(h, data);
+}
+
+int launch_fft_z_solve(dnslab *h, c2 *data)
+{
+    switch (h->P.nz) {
+    case 8: return launch_fft_z_solve_L<8>(h, data);
+    case 16: return launch_fft_z_solve_L<16>(h, data);
+    case 32: return launch_fft_z_solve_L<32>(h, data);
+    case 64: return launch_fft_z_solve_L<64>(h, data);
+    case 128: return launch_fft_z_solve_L<128>(h, data);
+    case 256: return launch_fft_z_solve_L<256>(h, data);
+    case 512: return launch_fft_z_solve_L<512>(h, data);
+    case 1024: return launch_fft_z_solve_L<1024>(h, data);
+    }
+    return DNSLAB_EINVAL;
+}
+
+// One solve p = F^-1[F[r]/lambda]; r = eq. 9 right-hand side built from (d, pold, face) on the fly
+// when `prologue`, else r = d as given.  pout may alias d or pold (it is written by the last pass).
+int poisson_solve(dnslab *h, const double *d, const double *pold, double *pout, bool prologue)
+{
+    dnsfft::PoissonRhsArgs ra;
+    ra.d = d; ra.p = pold; ra.face = (prologue ? h->face : nullptr);
+    ra.nx = h->P.nx; ra.ny = h->P.ny; ra.nz = h->P.nz;
+    ra.r2x = 1.0 / (2.0 * h->P.dx); ra.r2y = 1.0 / (2.0 * h->P.dy); ra.r2z = 1.0 / (2.0 * h->P.dz);
+    c2 *W = reinterpret_cast<c2 *>(h->W);
+    int rc;
+    if (prologue && h->face) rc = launch_fft_x<-1, true>(h, reinterpret_cast<const c2 *>(d), W, ra);
+    else rc = launch_fft_x<-1, false>(h, reinterpret_cast<const c2 *>(d), W, ra);
+    if (rc) return rc;
+    if ((rc = launch_fft_col<-1>(h, W, 1))) return rc;
+    if ((rc = launch_fft_z_solve(h, W))) return rc;
+    if ((rc = launch_fft_col<+1>(h, W, 1))) return rc;
+    return launch_fft_x<+1, false>(h, W, reinterpret_cast<c2 *>(pout), ra);
+}
+
+int launch_div(dnslab *h, double *const *q)
+{
+    const dim3 blk = tile_block(h);
+    const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz);
+    dnsst::k_div<<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], h->d, h->P.nx, h->P.ny, h->P.nz, 1.0 / (2.0 * h->P.dx),
+                                              1.0 / (2.0 * h->P.dy), 1.0 / (2.0 * h->P.dz));
+    return check_launch(h);
+}
+
+int launch_project(dnslab *h, double *const *q, const double *p)
+{
+    const dim3 blk = tile_block(h);
+    const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz);
+    const double r2x = 1.0 / (2.0 * h->P.dx), r2y = 1.0 / (2.0 * h->P.dy), r2z = 1.0 / (2.0 * h->P.dz);
+    if (h->face) dnsst::k_project<true><<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], p, h->face, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
+    else dnsst::k_project<false><<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], p, nullptr, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
+    return check_launch(h);
+}
+
+// divergence, n_piter iterations of eq. 9 warm-started from p, correction (in place on q)
+int pressure_stage(dnslab *h, double *const *q, double *p)
+{
+    int rc;
+    if ((rc = launch_div(h, q))) return rc;
+    for (int it = 0; it < h->P.n_piter; ++it)
+        if ((rc = poisson_solve(h, h->d, p, p, true))) return rc;
+    return launch_project(h, q, p);
+}
+
+} // namespace
+
+extern "C" {
+
+const char *dnslab_strerror(int code)
+{
+    switch (code) {
+    case DNSLAB_OK: return "ok";
+    case DNSLAB_EINVAL: return "invalid argument";
+    case DNSLAB_ENOMEM: return "workspace too small";
+    case DNSLAB_ECUDA: return "CUDA error";
+    case DNSLAB_EARCH: return "no sm_100 device";
+    }
+    return "unknown error";
+}
+
+size_t dnslab_workspace_bytes(const dnslab_params_t *params)
+{
+    if (!valid_params(params)) return 0;
+    return make_layout(params).total;
+}
+
+int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnslab_source_t *src, int32_t nsrc, void *workspace,
+                  void *cuda_stream, dnslab_t **out)
+{
+    if (!valid_params(params) || !workspace || !out || nsrc < 0 || nsrc > DNSLAB_MAX_SOURCES || (nsrc > 0 && !src)) return DNSLAB_EINVAL;
+    if ((uintptr_t)workspace % ALIGN) return DNSLAB_EINVAL;
+    for (int s = 0; s < nsrc; ++s)
+        if (!(src[s].tau_f > 0)) return DNSLAB_EINVAL;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return DNSLAB_EARCH;
+    if (prop.major != 10) return DNSLAB_EARCH;
+
+    dnslab *h = new (std::nothrow) dnslab;
+    if (!h) return DNSLAB_ENOMEM;
+    std::memset(h, 0, sizeof(*h));
+    h->P = *params;
+    h->n = (size_t)params->nx * params->ny * params->nz;
+    h->stream = (cudaStream_t)cuda_stream;
+    h->ws = (char *)workspace;
+    h->L = make_layout(params);
+    const Layout &L = h->L;
+    auto fld = [&](int idx) { return (double *)(h->ws + L.off_fields + (size_t)idx * L.field_bytes); };
+    for (int m = 0; m < 4; ++m) {
+        h->Q[m] = fld(m);
+        h->A[m] = fld(4 + m);
+        h->Bf[m] = fld(8 + m);
+        h->Qc[m] = fld(12 + m);
+    }
+    h->p = fld(16);
+    h->d = fld(17);
+    h->W = fld(18);
+    h->ps = (params->flags & 2u) ? fld(19) : nullptr;
+    h->zchunk = params->nz < 16 ? params->nz : 16;
+
+    auto fail = [&](int rc) { delete h; return rc; };
+#define CKF(call) do { if ((call) != cudaSuccess) return fail(DNSLAB_ECUDA); } while (0)
+    CKF(cudaMemsetAsync(h->ws + L.off_fields, 0, L.nfields * L.field_bytes, h->stream));
+
+    // mask -> face bytes; dropped entirely when there is no solid cell
+    h->face = nullptr;
+    if (mask) {
+        uint8_t *face = (uint8_t *)(h->ws + L.off_face);
+        uint8_t *tmp = (uint8_t *)h->W; // W is scratch here
+        CKF(cudaMemcpyAsync(tmp, mask, h->n, cudaMemcpyDefault, h->stream));
+        dim3 blk(params->nx < 128 ? params->nx : 128);
+        dim3 grd(params->nx / blk.x, params->ny, params->nz);
+        dnsst::k_face_mask<<<grd, blk, 0, h->stream>>>(tmp, face, params->nx, params->ny, params->nz);
+        h->launches++;
+        CKF(cudaPeekAtLastError());
+        std::vector<uint8_t> hm(h->n);
+        CKF(cudaMemcpyAsync(hm.data(), tmp, h->n, cudaMemcpyDeviceToHost, h->stream));
+        CKF(cudaStreamSynchronize(h->stream));
+        bool any_solid = false;
+        for (size_t o = 0; o < h->n; ++o)
+            if (!hm[o]) { any_solid = true; break; }
+        if (any_solid) h->face = face;
+        CKF(cudaMemsetAsync(h->W, 0, L.field_bytes, h->stream));
+    }
+
+    // twiddles exp(-2 pi i t/L) per axis and eigenvalue parts (sin(2 pi k/N_a)/D_a)^2
+    {
+        const int len[3] = {params->nx / 2, params->ny, params->nz};
+        const int full[3] = {params->nx, params->ny, params->nz};
+        const double dd[3] = {params->dx, params->dy, params->dz};
+        size_t eoff = 0;
+        for (int a = 0; a < 3; ++a) {
+            std::vector<c2> tw(len[a]);
+            for (int t = 0; t < len[a]; ++t) {
+                // exact octant reduction keeps the table symmetric and accurate to 0.5 ulp of libm
+                const long double ang = -2.0L * 3.141592653589793238462643383279502884L * (long double)t / (long double)len[a];
+                tw[t].x = (double)cosl(ang);
+                tw[t].y = (double)sinl(ang);
+            }
+            h->tw[a] = (c2 *)(h->ws + L.off_tw[a]);
+            CKF(cudaMemcpyAsync(h->tw[a], tw.data(), tw.size() * sizeof(c2), cudaMemcpyHostToDevice, h->stream));
+            std::vector<double> e(len[a]);
+            for (int k = 0; k < len[a]; ++k) {
+                const double s = std::sin(2.0 * M_PI * (double)k / (double)full[a]) / dd[a];
+                e[k] = s * s;
+            }
+            h->eig[a] = (double *)(h->ws + L.off_eig) + eoff;
+            eoff += len[a];
+            CKF(cudaMemcpyAsync(h->eig[a], e.data(), e.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+            CKF(cudaStreamSynchronize(h->stream));
+        }
+    }
+
+    // sources: one-dimensional factor tables of eq. 5
+    h->nsrc = nsrc;
+    h->stab = (double *)(h->ws + L.off_stab);
+    if (nsrc > 0) {
+        const int per = params->nx + params->ny + params->nz;
+        std::vector<double> tab((size_t)nsrc * per);
+        for (int s = 0; s < nsrc; ++s) {
+            double *t = tab.data() + (size_t)s * per;
+            source_profile(params->nx, params->dx, src[s].lo[0], src[s].size[0], src[s].B[0], t);
+            source_profile(params->ny, params->dy, src[s].lo[1], src[s].size[1], src[s].B[1], t + params->nx);
+            source_profile(params->nz, params->dz, src[s].lo[2], src[s].size[2], src[s].B[2], t + params->nx + params->ny);
+            dnsst::SourceDev &S = h->src[s];
+            for (int m = 0; m < 3; ++m) S.set[m] = src[s].u_set[m];
+            S.set[3] = src[s].c_set;
+            S.rtau = 1.0 / src[s].tau_f;
+            S.comps = src[s].comps & 0xF;
+            S.off = s * per;
+        }
+        CKF(cudaMemcpyAsync(h->stab, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+        CKF(cudaStreamSynchronize(h->stream));
+    }
+    CKF(cudaStreamSynchronize(h->stream));
+#undef CKF
+    *out = h;
+    return DNSLAB_OK;
+}
+
+int dnslab_set_fields(dnslab_t *h, const double *u, const double *v, const double *w, const double *c, const double *p)
+{
+    if (!h || !u || !v || !w || !c) return DNSLAB_EINVAL;
+    const double *in[4] = {u, v, w, c};
+    const size_t bytes = h->n * sizeof(double);
+    for (int m = 0; m < 4; ++m) CK(cudaMemcpyAsync(h->Q[m], in[m], bytes, cudaMemcpyDefault, h->stream));
+    if (p) CK(cudaMemcpyAsync(h->p, p, bytes, cudaMemcpyDefault, h->stream));
+    else CK(cudaMemsetAsync(h->p, 0, bytes, h->stream));
+    if (h->face) {
+        dnsst::k_mask_select<<<(unsigned)((h->n + 255) / 256), 256, 0, h->stream>>>(h->Q[0], h->Q[1], h->Q[2], h->Q[3], h->face, h->n);
+        return check_launch(h);
+    }
+    return DNSLAB_OK;
+}
+
+int dnslab_step(dnslab_t *h, int32_t nsteps)
+{
+    if (!h || nsteps < 0) return DNSLAB_EINVAL;
+    const bool stage_proj = (h->P.flags & 2u) != 0;
+    const size_t bytes = h->n * sizeof(double);
+    int rc;
+    for (int it = 0; it < nsteps; ++it) {
+        if ((rc = launch_rk<1>(h, h->Q, h->A))) return rc;
+        if (stage_proj) {
+            CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
+            if ((rc = pressure_stage(h, h->A, h->ps))) return rc;
+        }
+        if ((rc = launch_rk<2>(h, h->A, h->Bf))) return rc;
+        if (stage_proj) {
+            CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
+            if ((rc = pressure_stage(h, h->Bf, h->ps))) return rc;
+        }
+        if ((rc = launch_rk<3>(h, h->Bf, h->A))) return rc;
+        if (stage_proj) {
+            CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
+            if ((rc = pressure_stage(h, h->A, h->ps))) return rc;
+        }
+        if ((rc = launch_rk<4>(h, h->A, nullptr))) return rc;
+        if ((rc = pressure_stage(h, h->Qc, h->p))) return rc;
+        for (int m = 0; m < 4; ++m) {
+            double *t = h->Q[m];
+            h->Q[m] = h->Qc[m];
+            h->Qc[m] = t;
+        }
+    }
+    return DNSLAB_OK;
+}
+
+int dnslab_poisson(dnslab_t *h, const double *rhs, double *p)
+{
+    if (!h || !rhs || !p) return DNSLAB_EINVAL;
+    return poisson_solve(h, rhs, nullptr, p, false);
+}
+
+int dnslab_fields(dnslab_t *h, const double **u, const double **v, const double **w, const double **c, const double **p)
+{
+    if (!h) return DNSLAB_EINVAL;
+    if (u) *u = h->Q[0];
+    if (v) *v = h->Q[1];
+    if (w) *w = h->Q[2];
+    if (c) *c = h->Q[3];
+    if (p) *p = h->p;
+    return DNSLAB_OK;
+}
+
+int dnslab_get_fields(dnslab_t *h, double *u, double *v, double *w, double *c, double *p)
+{
+    if (!h) return DNSLAB_EINVAL;
+    double *out[5] = {u, v, w, c, p};
+    const double *in[5] = {h->Q[0], h->Q[1], h->Q[2], h->Q[3], h->p};
+    for (int m = 0; m < 5; ++m)
+        if (out[m]) CK(cudaMemcpyAsync(out[m], in[m], h->n * sizeof(double), cudaMemcpyDefault, h->stream));
+    return DNSLAB_OK;
+}
+
+int64_t dnslab_launch_count(const dnslab_t *h) { return h ? h->launches : -1; }
+
+int dnslab_destroy(dnslab_t *h)
+{
+    if (!h) return DNSLAB_EINVAL;
+    delete h;
+    return DNSLAB_OK;
+}
+
+} // extern "C"

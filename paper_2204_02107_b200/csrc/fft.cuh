@@ -1,0 +1,283 @@
+// fft.cuh -- hand-written fp64 complex FFT passes for the pressure Poisson solve (eq. 9).
+//
+// The solve works on the real nx*ny*nz array reinterpreted as (nx/2)*ny*nz complex numbers
+// (even cell -> re, odd cell -> im).  The operator sum_a delta_a delta_a only couples cells two
+// apart, so even and odd x-sublattices are independent real problems and one complex-to-complex
+// transform of half length in x solves both.
+//
+// Every pass is a Stockham autosort FFT held in registers (E elements per thread, radix-8/4/2
+// butterflies) with shared-memory exchanges between radix stages.  Thread `tid` of a line always
+// owns elements tid + e*T (T = L/E), both on entry and on exit, so the first stage reads global
+// memory directly and the last stage writes it directly; the fused z pass keeps the spectrum in
+// registers between the forward and the inverse transform.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace dnsfft {
+
+typedef double2 c2;
+
+__device__ __forceinline__ c2 cadd(c2 a, c2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ c2 csub(c2 a, c2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ c2 cmul(c2 a, c2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+// multiply by -i (forward quarter turn) or +i (inverse)
+template <int DIR> __device__ __forceinline__ c2 rot90(c2 a)
+{
+    return DIR < 0 ? make_double2(a.y, -a.x) : make_double2(-a.y, a.x);
+}
+// multiply by the table twiddle w = exp(-2 pi i t/L) (forward) or its conjugate (inverse)
+template <int DIR> __device__ __forceinline__ c2 twmul(c2 a, c2 w)
+{
+    return DIR < 0 ? make_double2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x)
+                   : make_double2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y);
+}
+
+template <int DIR> __device__ __forceinline__ void dft2(c2 &a, c2 &b)
+{
+    c2 t = a;
+    a = cadd(t, b);
+    b = csub(t, b);
+}
+
+template <int DIR> __device__ __forceinline__ void dft4(c2 &a0, c2 &a1, c2 &a2, c2 &a3)
+{
+    c2 t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), t3 = rot90<DIR>(csub(a1, a3));
+    a0 = cadd(t0, t2);
+    a2 = csub(t0, t2);
+    a1 = cadd(t1, t3);
+    a3 = csub(t1, t3);
+}
+
+template <int DIR> __device__ __forceinline__ void dft8(c2 (&v)[8])
+{
+    const double h = 0.70710678118654752440;
+    // even and odd 4-point transforms
+    dft4<DIR>(v[0], v[2], v[4], v[6]);
+    dft4<DIR>(v[1], v[3], v[5], v[7]);
+    // odd outputs times w8^k, k = 1,2,3:  forward w8 = (1 - i)/sqrt2
+    c2 o1 = DIR < 0 ? make_double2((v[3].x + v[3].y) * h, (v[3].y - v[3].x) * h)
+                    : make_double2((v[3].x - v[3].y) * h, (v[3].y + v[3].x) * h);
+    c2 o2 = rot90<DIR>(v[5]);
+    c2 o3 = DIR < 0 ? make_double2((v[7].y - v[7].x) * h, -(v[7].x + v[7].y) * h)
+                    : make_double2(-(v[7].x + v[7].y) * h, (v[7].x - v[7].y) * h);
+    c2 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
+    v[0] = cadd(e0, o0);
+    v[4] = csub(e0, o0);
+    v[1] = cadd(e1, o1);
+    v[5] = csub(e1, o1);
+    v[2] = cadd(e2, o2);
+    v[6] = csub(e2, o2);
+    v[3] = cadd(e3, o3);
+    v[7] = csub(e3, o3);
+}
+
+// One Stockham stage of radix R on the E register elements of thread `tid` (element e <-> index
+// tid + e*T).  Ns = product of the radices of the earlier stages.  On exit slot q + r*(E/R) holds
+// output r of butterfly jj = tid + q*T, whose natural position is oidx = expand(jj) + r*Ns.
+template <int L, int E, int R, int NS, int DIR> __device__ __forceinline__ void stage(c2 (&x)[E], int tid, const c2 *__restrict__ tw)
+{
+    constexpr int T = L / E;
+    constexpr int Q = E / R;
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+        c2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = x[q + r * Q];
+        if constexpr (NS > 1) {
+            const int jm = (tid + q * T) & (NS - 1);
+            const int kb = jm * (L / (NS * R));
+#pragma unroll
+            for (int r = 1; r < R; ++r) v[r] = twmul<DIR>(v[r], __ldg(&tw[kb * r]));
+        }
+        if constexpr (R == 8) {
+            dft8<DIR>(v);
+        } else if constexpr (R == 4) {
+            dft4<DIR>(v[0], v[1], v[2], v[3]);
+        } else if constexpr (R == 2) {
+            dft2<DIR>(v[0], v[1]);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) x[q + r * Q] = v[r];
+    }
+}
+
+template <int L, int E, int NS> struct NextRadix {
+    static constexpr int rem = L / NS;
+    static constexpr int value = rem >= 8 ? (E >= 8 ? 8 : E) : rem;
+};
+
+// Full transform of one line held as x[e] <-> element tid + e*T, exchanging through `sm`
+// (SM::at(n) gives a reference to the shared slot of logical element n of this thread's line).
+// All threads of the block must call this together (it contains __syncthreads()).
+template <int L, int E, int DIR, int NS, class SM> __device__ __forceinline__ void fft_line(c2 (&x)[E], int tid, const c2 *__restrict__ tw, SM &sm)
+{
+    constexpr int T = L / E;
+    constexpr int R = NextRadix<L, E, NS>::value;
+    constexpr int Q = E / R;
+    stage<L, E, R, NS, DIR>(x, tid, tw);
+    if constexpr (NS * R < L) {
+#pragma unroll
+        for (int q = 0; q < Q; ++q) {
+            const int jj = tid + q * T;
+            const int jm = jj & (NS - 1);
+            const int j0 = (jj - jm) * R + jm;
+#pragma unroll
+            for (int r = 0; r < R; ++r) sm.at(j0 + r * NS) = x[q + r * Q];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = sm.at(tid + e * T);
+        __syncthreads();
+        fft_line<L, E, DIR, NS * R, SM>(x, tid, tw, sm);
+    }
+}
+
+// shared-memory views -------------------------------------------------------------------
+// contiguous line with one pad element per 8 (x pass: threads of a warp walk along the line)
+struct SmLine {
+    c2 *base;
+    __device__ __forceinline__ c2 &at(int n) { return base[n + (n >> 3)]; }
+};
+// column of a tile whose fastest index is the XT-wide x offset (y and z passes)
+template <int XT> struct SmCol {
+    c2 *base; // already offset by tx
+    __device__ __forceinline__ c2 &at(int n) { return base[n * XT]; }
+};
+
+template <int L> struct ElemsPerThread { static constexpr int value = L >= 8 ? 8 : L; };
+
+// ---------------------------------------------------------------------------------------
+// Right-hand side of eq. 9 at one cell: r = d + sum_a delta_a[(1-beta) delta_a p].
+// face: bit0 beta(cell), bit1/2 beta(x+1/x-1), bit3/4 beta(y+1/y-1), bit5/6 beta(z+1/z-1).
+// (1-beta) is 0 in the fluid, so the bracket needs p only next to solid cells.
+struct PoissonRhsArgs {
+    const double *d;
+    const double *p;
+    const uint8_t *face; // null: beta == 1 everywhere
+    int nx, ny, nz;
+    double r2x, r2y, r2z; // 1/(2 D_a)
+};
+
+__device__ __forceinline__ double eq9_rhs(const PoissonRhsArgs &a, double dv, int i, int j, int k, unsigned f)
+{
+    if ((f & 0x7e) == 0x7e) return dv; // all six neighbours fluid: bracket is exactly 0
+    const int nx = a.nx, ny = a.ny, nz = a.nz;
+    const size_t row = (size_t)nx * ((size_t)j + (size_t)ny * k);
+    const double *p = a.p;
+    const double pc = __ldg(&p[row + i]);
+    double gxp = 0.0, gxm = 0.0, gyp = 0.0, gym = 0.0, gzp = 0.0, gzm = 0.0;
+    if (!(f & 2)) gxp = (__ldg(&p[row + ((i + 2) & (nx - 1))]) - pc) * a.r2x;
+    if (!(f & 4)) gxm = (pc - __ldg(&p[row + ((i - 2) & (nx - 1))])) * a.r2x;
+    if (!(f & 8)) gyp = (__ldg(&p[(size_t)nx * ((size_t)((j + 2) & (ny - 1)) + (size_t)ny * k) + i]) - pc) * a.r2y;
+    if (!(f & 16)) gym = (pc - __ldg(&p[(size_t)nx * ((size_t)((j - 2) & (ny - 1)) + (size_t)ny * k) + i])) * a.r2y;
+    if (!(f & 32)) gzp = (__ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k + 2) & (nz - 1))) + i]) - pc) * a.r2z;
+    if (!(f & 64)) gzm = (pc - __ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k - 2) & (nz - 1))) + i])) * a.r2z;
+    return dv + ((gxp - gxm) * a.r2x + (gyp - gym) * a.r2y + (gzp - gzm) * a.r2z);
+}
+
+// ---------------------------------------------------------------------------------------
+// x pass: lines of L = nx/2 complex numbers, contiguous.  NL lines per block.
+//   FWD with PROLOGUE: in = d (real array viewed as complex), r = eq9_rhs(...) computed on load.
+//   out-of-place or in-place (a block reads its lines completely before it writes them).
+template <int L, int DIR, bool PROLOGUE>
+__global__ void __launch_bounds__(256) k_fft_x(const c2 *__restrict__ in, c2 *__restrict__ out, const c2 *__restrict__ tw, int nlines_per_block,
+                                               PoissonRhsArgs ra)
+{
+    constexpr int E = ElemsPerThread<L>::value;
+    constexpr int T = L / E;
+    extern __shared__ double2 smem[];
+    const int lt = threadIdx.x / T; // line within block
+    const int tid = threadIdx.x - lt * T;
+    const size_t line = (size_t)blockIdx.x * nlines_per_block + lt;
+    const c2 *src = in + line * L;
+    c2 x[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) x[e] = src[tid + e * T];
+    if (PROLOGUE) {
+        if (ra.face != nullptr) {
+            const int j = (int)(line % ra.ny), k = (int)(line / ra.ny);
+            const uint8_t *frow = ra.face + line * (size_t)(2 * L);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int m = tid + e * T;
+                const uchar2 f = *reinterpret_cast<const uchar2 *>(frow + 2 * m);
+                x[e].x = eq9_rhs(ra, x[e].x, 2 * m, j, k, f.x);
+                x[e].y = eq9_rhs(ra, x[e].y, 2 * m + 1, j, k, f.y);
+            }
+        }
+    }
+    SmLine sm{smem + lt * (L + L / 8)};
+    fft_line<L, E, DIR, 1, SmLine>(x, tid, tw, sm);
+    c2 *dst = out + line * L;
+#pragma unroll
+    for (int e = 0; e < E; ++e) dst[tid + e * T] = x[e];
+}
+
+// y or z pass, in place: XT adjacent x (complex) by L elements along the axis; element n of
+// column tx is at base + n*stride + tx.  blockIdx.x enumerates (x tile, other index).
+template <int L, int XT, int DIR>
+__global__ void __launch_bounds__(XT *(L / ElemsPerThread<L>::value) < 32 ? 32 : XT *(L / ElemsPerThread<L>::value))
+    k_fft_col(c2 *__restrict__ data, const c2 *__restrict__ tw, int mx, size_t stride, size_t other_stride)
+{
+    constexpr int E = ElemsPerThread<L>::value;
+    constexpr int T = L / E;
+    extern __shared__ double2 smem[];
+    const int tx = threadIdx.x % XT;
+    const int tid = threadIdx.x / XT;
+    const int xtiles = mx / XT;
+    const int xt = blockIdx.x % xtiles;
+    const size_t other = blockIdx.x / xtiles;
+    c2 *base = data + other * other_stride + (size_t)xt * XT + tx;
+    c2 x[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) x[e] = base[(size_t)(tid + e * T) * stride];
+    SmCol<XT> sm{smem + tx};
+    fft_line<L, E, DIR, 1, SmCol<XT>>(x, tid, tw, sm);
+#pragma unroll
+    for (int e = 0; e < E; ++e) base[(size_t)(tid + e * T) * stride] = x[e];
+}
+
+// Fused middle pass along z: forward transform, division by the modified-wavenumber eigenvalue
+//   lambda(m,ky,kz) = -(ex[m] + ey[ky] + ez[kz]),  e_a[k] = (sin(2 pi k/N_a)/D_a)^2,
+// null modes (m = 0, 2ky = 0 mod ny, 2kz = 0 mod nz) set to 0, scaling by 1/N, inverse transform.
+// blockIdx.x enumerates (x tile, ky).
+template <int L, int XT>
+__global__ void __launch_bounds__(XT *(L / ElemsPerThread<L>::value) < 32 ? 32 : XT *(L / ElemsPerThread<L>::value))
+    k_fft_z_solve(c2 *__restrict__ data, const c2 *__restrict__ tw, int mx, int ny, const double *__restrict__ ex,
+                  const double *__restrict__ ey, const double *__restrict__ ez, double inv_n)
+{
+    constexpr int E = ElemsPerThread<L>::value;
+    constexpr int T = L / E;
+    extern __shared__ double2 smem[];
+    const int tx = threadIdx.x % XT;
+    const int tid = threadIdx.x / XT;
+    const int xtiles = mx / XT;
+    const int xt = blockIdx.x % xtiles;
+    const int ky = blockIdx.x / xtiles;
+    const int m = xt * XT + tx;
+    const size_t stride = (size_t)mx * ny;
+    c2 *base = data + (size_t)ky * mx + m;
+    c2 x[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) x[e] = base[(size_t)(tid + e * T) * stride];
+    SmCol<XT> sm{smem + tx};
+    fft_line<L, E, -1, 1, SmCol<XT>>(x, tid, tw, sm);
+    const double exy = __ldg(&ex[m]) + __ldg(&ey[ky]);
+    const bool null_xy = (m == 0) && (((2 * ky) & (ny - 1)) == 0);
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int kz = tid + e * T;
+        const double lam = -(exy + __ldg(&ez[kz]));
+        const bool null = null_xy && (((2 * kz) & (L - 1)) == 0);
+        const double s = null ? 0.0 : inv_n / lam;
+        x[e].x = null ? 0.0 : x[e].x * s;
+        x[e].y = null ? 0.0 : x[e].y * s;
+    }
+    __syncthreads();
+    fft_line<L, E, +1, 1, SmCol<XT>>(x, tid, tw, sm);
+#pragma unroll
+    for (int e = 0; e < E; ++e) base[(size_t)(tid + e * T) * stride] = x[e];
+}
+
+} // namespace dnsfft

@@ -1,0 +1,231 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's: per-field max|a-b|/max|b| <= 1e-11 after one
+step, <= 1e-8 after 100 steps; solid cells bit-exact +0.0."""
+import numpy as np
+import pytest
+
+from conftest import relerr
+from oracle import dnsref
+from paper_2204_02107_b200 import binding, cases
+
+pytestmark = pytest.mark.gpu
+
+TOL1, TOL100 = 1e-11, 1e-8
+
+
+def oracle_for(case, n_piter=None, flags=0):
+    o = dnsref.Oracle(case["shape"], case["d"], case["nu"], case["alpha_c"], case["dt"], mask=case["mask"],
+                      sources=case["sources"], body=case["body"], n_piter=n_piter or case["n_piter"], flags=flags)
+    o.set_fields(case["u"], case["v"], case["w"], case["c"])
+    return o
+
+
+def compare(got, ref, tol, mask=None, what=""):
+    for k in "uvwcp":
+        e = relerr(got[k], ref[k])
+        assert e <= tol, (what, k, e)
+    if mask is not None:
+        solid = mask == 0
+        for k in "uvwc":
+            assert np.all(got[k][solid] == 0.0) and not np.any(np.signbit(got[k][solid])), (what, k)
+
+
+def run_both(case, checkpoints, n_piter=None, flags=0):
+    s = binding.solver_for_case(case, n_piter=n_piter, flags=flags)
+    o = oracle_for(case, n_piter=n_piter, flags=flags)
+    done = 0
+    for cp in checkpoints:
+        s.step(cp - done)
+        o.step(cp - done)
+        done = cp
+        yield cp, s.fields_numpy(), o.fields()
+    s.close()
+    o.close()
+
+
+# ------------------------------------------------------------------ Poisson solve alone
+@pytest.mark.parametrize("shape", [(8, 8, 8), (8, 16, 32), (32, 8, 16), (16, 32, 64), (64, 32, 128), (32, 128, 256),
+                                   (128, 64, 16), (8, 8, 512), (8, 8, 1024), (8, 8, 2048), (8, 512, 8), (8, 1024, 16),
+                                   (256, 8, 8), (512, 8, 16), (1024, 8, 8)])
+def test_poisson_matches_oracle(shape):
+    import torch
+    rng = np.random.default_rng(sum(shape))
+    d = (0.11, 0.07, 0.05)
+    rhs = rng.standard_normal(shape)
+    s = binding.Solver(shape, d, 0.1, 0.1, 0.1)
+    p = s.poisson(torch.from_numpy(rhs).cuda())
+    # in place too
+    buf = torch.from_numpy(rhs).cuda()
+    s.poisson(buf, out=buf)
+    s.synchronize()
+    o = dnsref.Oracle(shape, d, 0.1, 0.1, 0.1)
+    ref = o.poisson(rhs)
+    assert relerr(p.cpu().numpy(), ref) <= 1e-13 * max(1, np.log2(max(shape)))
+    assert torch.equal(buf, p)
+
+
+def test_poisson_null_modes_and_manufactured():
+    import torch
+    shape, d = (16, 32, 64), (0.2, 0.3, 0.25)
+    nz, ny, nx = shape
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    s = binding.Solver(shape, d, 0.1, 0.1, 0.1)
+    # a right-hand side made only of the 8 null modes solves to exactly zero
+    null = 1.0 + (-1.0) ** i + 0.5 * (-1.0) ** (j + k) + 0.25 * (-1.0) ** (i + j + k)
+    p = s.poisson(torch.from_numpy(null).cuda()).cpu().numpy()
+    assert np.abs(p).max() < 1e-13
+    pm = np.cos(2 * np.pi * 5 * i / nx + 0.3) * np.cos(2 * np.pi * 3 * j / ny) * np.cos(2 * np.pi * 7 * k / nz - 0.2)
+    lam = -(np.sin(2 * np.pi * 5 / nx) ** 2 / d[0] ** 2 + np.sin(2 * np.pi * 3 / ny) ** 2 / d[1] ** 2 +
+            np.sin(2 * np.pi * 7 / nz) ** 2 / d[2] ** 2)
+    p = s.poisson(torch.from_numpy(lam * pm).cuda()).cpu().numpy()
+    assert np.abs(p - pm).max() < 1e-13
+
+
+# ------------------------------------------------------------------ full step, the five configs
+def test_config1_taylor_green_10_steps():
+    case = cases.config(1)
+    E0 = sum((case[k] ** 2).sum() for k in "uvw")
+    gold = {1: 0.99544004, 10: 0.95539285}   # tests/golden/tgv32_energy.txt
+    for cp, got, ref in run_both(case, [1, 10]):
+        compare(got, ref, TOL1 if cp == 1 else TOL100, what=f"tgv step {cp}")
+        E = sum((got[k] ** 2).sum() for k in "uvw") / E0
+        assert abs(E - gold[cp]) < 5e-8
+
+
+@pytest.mark.parametrize("n_piter", [4, 1])
+def test_config2_duct_room_100_steps(n_piter):
+    case = cases.config(2)
+    for cp, got, ref in run_both(case, [1, 100], n_piter=n_piter):
+        compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"duct P={n_piter} step {cp}")
+
+
+def test_config3_periodic_turbulence_64_100_steps():
+    case = cases.config(3, shrink=4)
+    for cp, got, ref in run_both(case, [1, 100]):
+        compare(got, ref, TOL1 if cp == 1 else TOL100, what=f"turb64 step {cp}")
+
+
+def test_config4_room_quarter_size_100_steps():
+    case = cases.config(4, shrink=4)
+    for cp, got, ref in run_both(case, [1, 100]):
+        compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"room/4 step {cp}")
+
+
+def test_config5_three_rooms_eighth_size_20_steps():
+    case = cases.config(5, shrink=8)
+    for cp, got, ref in run_both(case, [1, 20]):
+        compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"rooms/8 step {cp}")
+
+
+@pytest.mark.slow
+def test_config3_full_size_one_step():
+    case = cases.config(3)
+    for cp, got, ref in run_both(case, [1]):
+        compare(got, ref, TOL1, what="turb256 step 1")
+
+
+@pytest.mark.slow
+def test_config4_full_size_one_step():
+    case = cases.config(4)
+    for cp, got, ref in run_both(case, [1]):
+        compare(got, ref, TOL1, mask=case["mask"], what="room512 step 1")
+
+
+# ------------------------------------------------------------------ variants and edge cases
+def test_per_stage_projection_variant():
+    case = cases.duct_room(32, 16, 16)
+    for cp, got, ref in run_both(case, [1, 5], flags=2):
+        compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"flags=2 step {cp}")
+
+
+def test_smooth_tanh_sources_and_body_force_unequal_spacing():
+    case = cases.duct_room(32, 16, 16)
+    case["d"] = (0.05, 0.07, 0.06)
+    case["body"] = (1e-3, -2e-3, 5e-4)
+    case["sources"] = [dict(case["sources"][0], B=(3.0, 2.0, 0.0), comps=0b1011),
+                       dict(lo=(10, 4, 5), size=(5, 4, 3), B=(0.0, 4.0, 2.5), u_set=(0.0, 0.05, -0.02), c_set=0.5,
+                            tau_f=3 * case["dt"], comps=0b1110)]
+    for cp, got, ref in run_both(case, [1, 10]):
+        compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"tanh sources step {cp}")
+
+
+def test_smallest_grid_and_degenerate_masks():
+    rng = np.random.default_rng(3)
+    shape = (8, 8, 8)
+    base = dict(shape=shape, d=(0.3, 0.2, 0.25), nu=0.01, alpha_c=0.02, dt=0.01, body=(0.0, 0.0, 0.0), n_piter=2,
+                sources=[], u=rng.standard_normal(shape), v=rng.standard_normal(shape), w=rng.standard_normal(shape),
+                c=rng.standard_normal(shape))
+    # explicit all-fluid mask == no mask
+    for mask in (None, np.ones(shape, np.uint8)):
+        case = dict(base, mask=mask)
+        for cp, got, ref in run_both(case, [1, 3]):
+            compare(got, ref, TOL1, what="8^3")
+    # all solid: everything stays exactly zero
+    case = dict(base, mask=np.zeros(shape, np.uint8))
+    for cp, got, ref in run_both(case, [2]):
+        for k in "uvwcp":
+            assert np.all(got[k] == 0.0) and np.all(ref[k] == 0.0)
+    # a single solid cell, and a single fluid cell
+    m1 = np.ones(shape, np.uint8); m1[3, 4, 5] = 0
+    m2 = np.zeros(shape, np.uint8); m2[3, 4, 5] = 1
+    for mask in (m1, m2):
+        case = dict(base, mask=mask)
+        for cp, got, ref in run_both(case, [1, 3]):
+            compare(got, ref, TOL1, mask=mask, what="single cell mask")
+
+
+def test_anisotropic_long_grids():
+    rng = np.random.default_rng(8)
+    for shape in [(8, 8, 256), (8, 128, 8), (64, 8, 16)]:
+        mask = (rng.random(shape) > 0.1).astype(np.uint8)
+        case = dict(shape=shape, d=(0.1, 0.12, 0.09), nu=0.01, alpha_c=0.01, dt=0.004, body=(0.0, 0.0, 0.0), n_piter=3,
+                    mask=mask, sources=[], u=0.3 * rng.standard_normal(shape), v=0.3 * rng.standard_normal(shape),
+                    w=0.3 * rng.standard_normal(shape), c=rng.standard_normal(shape))
+        for cp, got, ref in run_both(case, [1, 4]):
+            compare(got, ref, TOL1, mask=mask, what=f"{shape}")
+
+
+def test_device_inputs_borrowed_pointers_and_warm_start_pressure():
+    import torch
+    case = cases.duct_room(32, 16, 16)
+    dev = {k: torch.from_numpy(case[k]).cuda() for k in "uvwc"}
+    p0 = np.random.default_rng(5).standard_normal(case["shape"]) * 1e-3
+    s = binding.Solver(case["shape"], case["d"], case["nu"], case["alpha_c"], case["dt"],
+                       mask=torch.from_numpy(case["mask"]).cuda(), sources=case["sources"], n_piter=4)
+    s.set_fields(dev["u"], dev["v"], dev["w"], dev["c"], torch.from_numpy(p0).cuda())
+    s.step(1)
+    got = s.fields_numpy()
+    o = oracle_for(case)
+    o.set_fields(case["u"], case["v"], case["w"], case["c"], p0)
+    o.step(1)
+    compare(got, o.fields(), TOL1, mask=case["mask"], what="device inputs")
+    ptrs = s.field_ptrs()
+    assert all(ptrs[k] for k in "uvwcp") and len(set(ptrs.values())) == 5
+    n0 = s.launch_count()
+    s.step(1)
+    assert s.launch_count() - n0 == 4 + 1 + 5 * 4 + 1   # 4 RK stages, div, 4 x 5 FFT passes, projection
+    # host output buffers
+    out = {k: np.empty(case["shape"]) for k in "uvwcp"}
+    s.get_fields(**out)
+    s.synchronize()
+    o.step(1)
+    compare(out, o.fields(), TOL1, mask=case["mask"], what="host outputs")
+
+
+def test_create_rejects_bad_arguments():
+    import ctypes as C
+    import torch
+    L = binding.lib()
+    P = binding.make_params((8, 8, 8), (1, 1, 1), 0.1, 0.1, 0.1)
+    ws = torch.empty(binding.workspace_bytes(P) + 512, dtype=torch.uint8, device="cuda")
+    base = (ws.data_ptr() + 255) // 256 * 256
+    h = C.c_void_p()
+    assert L.dnslab_create(C.byref(P), None, None, 0, base + 8, None, C.byref(h)) == -1      # misaligned
+    assert L.dnslab_create(C.byref(P), None, None, 0, None, None, C.byref(h)) == -1          # null workspace
+    assert L.dnslab_create(C.byref(P), None, None, 3, base, None, C.byref(h)) == -1          # nsrc without src
+    bad = binding.make_sources([dict(lo=(0, 0, 0), size=(1, 1, 1), tau_f=0.0)])
+    assert L.dnslab_create(C.byref(P), None, bad, 1, base, None, C.byref(h)) == -1           # tau_f <= 0
+    assert L.dnslab_create(C.byref(P), None, None, 0, base, None, C.byref(h)) == 0
+    assert L.dnslab_step(h, -1) == -1
+    assert L.dnslab_poisson(h, None, None) == -1
+    assert L.dnslab_destroy(h) == 0
