@@ -234,7 +234,7 @@ template <int L, int XT> int launch_fft_z_solve_LX(dnslab *h, c2 *data)
     const size_t smem = (size_t)XT * L * sizeof(c2);
     auto kern = dnsfft::k_fft_z_solve<L, XT>;
     if (int rc = set_smem(kern, smem)) return rc;
-    const double inv_n = 1.0 / (double)h->n;
+    const double inv_n = 2.0 / (double)h->n; // the packed transform has n/2 complex points
     kern<<<(unsigned)((mx / XT) * h->P.ny), XT * T, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], inv_n);
     return check_launch(h);
 }
