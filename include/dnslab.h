@@ -107,6 +107,21 @@ int dnslab_get_fields(dnslab_t *h, double *u, double *v, double *w, double *c, d
 /* Number of kernels the library has launched on this handle since create (for bench accounting). */
 int64_t dnslab_launch_count(const dnslab_t *h);
 
+/* Per-kernel timing (measurement aid; off by default).  While enabled every kernel launch is
+ * bracketed by CUDA events on the solver's stream and accounted to one of these classes.
+ * dnslab_profile(h, 1) clears the totals and starts; dnslab_profile(h, 0) stops.
+ * dnslab_profile_read synchronises the stream and writes, per class, the summed device time in
+ * milliseconds and the number of launches into two host arrays of DNSLAB_NCLASS entries. */
+#define DNSLAB_K_RK 0      /* fused RHS + Runge-Kutta stage kernel (4 per step)            */
+#define DNSLAB_K_DIV 1     /* divergence                                                   */
+#define DNSLAB_K_FFT_X 2   /* x-axis FFT passes (forward with the eq. 9 prologue, inverse) */
+#define DNSLAB_K_FFT_Y 3   /* y-axis FFT passes                                            */
+#define DNSLAB_K_FFT_Z 4   /* fused z forward + eigenvalue division + z inverse pass       */
+#define DNSLAB_K_PROJECT 5 /* pressure-gradient projection                                 */
+#define DNSLAB_NCLASS 6
+int dnslab_profile(dnslab_t *h, int enable);
+int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches);
+
 int dnslab_destroy(dnslab_t *h);
 
 const char *dnslab_strerror(int code);

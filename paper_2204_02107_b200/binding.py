@@ -11,7 +11,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdnslab.so")
 
 SYMBOLS = ["dnslab_workspace_bytes", "dnslab_create", "dnslab_set_fields", "dnslab_step", "dnslab_poisson",
-           "dnslab_fields", "dnslab_get_fields", "dnslab_launch_count", "dnslab_destroy", "dnslab_strerror"]
+           "dnslab_fields", "dnslab_get_fields", "dnslab_launch_count", "dnslab_profile", "dnslab_profile_read",
+           "dnslab_destroy", "dnslab_strerror"]
+KERNEL_CLASSES = ["rk_stage", "div", "fft_x", "fft_y", "fft_z_solve", "project"]
 
 
 class Params(C.Structure):
@@ -53,6 +55,8 @@ def lib():
         L.dnslab_get_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 5
         L.dnslab_launch_count.argtypes = [C.c_void_p]
         L.dnslab_launch_count.restype = C.c_int64
+        L.dnslab_profile.argtypes = [C.c_void_p, C.c_int]
+        L.dnslab_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.dnslab_destroy.argtypes = [C.c_void_p]
         L.dnslab_strerror.argtypes = [C.c_int]
         L.dnslab_strerror.restype = C.c_char_p
@@ -163,6 +167,16 @@ class Solver:
 
     def launch_count(self):
         return int(lib().dnslab_launch_count(self._h))
+
+    def profile(self, enable):
+        _check(lib().dnslab_profile(self._h, int(bool(enable))), "dnslab_profile")
+
+    def profile_read(self):
+        """{class: (total ms, launches)} since profile(True)."""
+        n = len(KERNEL_CLASSES)
+        ms, cnt = (C.c_double * n)(), (C.c_int64 * n)()
+        _check(lib().dnslab_profile_read(self._h, ms, cnt), "dnslab_profile_read")
+        return {k: (ms[i], int(cnt[i])) for i, k in enumerate(KERNEL_CLASSES)}
 
     # -- conveniences (marshalling only) ---------------------------------------------------
     def fields(self):

@@ -79,6 +79,11 @@ void source_profile(int n, double d, int lo, int size, double B, double *out)
 
 } // namespace
 
+struct ProfRec {
+    int cls;
+    cudaEvent_t e0, e1;
+};
+
 struct dnslab {
     dnslab_params_t P;
     size_t n;
@@ -94,6 +99,11 @@ struct dnslab {
     dnsst::SourceDev src[DNSLAB_MAX_SOURCES];
     int64_t launches;
     int zchunk;
+    // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
+    bool prof_on;
+    std::vector<ProfRec> *prof;
+    double prof_ms[DNSLAB_NCLASS];
+    int64_t prof_n[DNSLAB_NCLASS];
 };
 
 namespace {
@@ -103,6 +113,45 @@ namespace {
         cudaError_t e_ = (call);                   \
         if (e_ != cudaSuccess) return DNSLAB_ECUDA; \
     } while (0)
+
+// Accumulate finished event pairs into the per-class totals (synchronises the stream).
+int prof_drain(dnslab *h)
+{
+    if (!h->prof || h->prof->empty()) return DNSLAB_OK;
+    CK(cudaStreamSynchronize(h->stream));
+    for (ProfRec &r : *h->prof) {
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, r.e0, r.e1));
+        h->prof_ms[r.cls] += ms;
+        h->prof_n[r.cls] += 1;
+        cudaEventDestroy(r.e0);
+        cudaEventDestroy(r.e1);
+    }
+    h->prof->clear();
+    return DNSLAB_OK;
+}
+
+// Brackets one kernel launch with events when profiling is on.
+struct ProfScope {
+    dnslab *h;
+    ProfRec r;
+    bool on;
+    ProfScope(dnslab *h_, int cls) : h(h_), on(h_->prof_on)
+    {
+        if (!on) return;
+        r.cls = cls;
+        cudaEventCreate(&r.e0);
+        cudaEventCreate(&r.e1);
+        cudaEventRecord(r.e0, h->stream);
+    }
+    ~ProfScope()
+    {
+        if (!on) return;
+        cudaEventRecord(r.e1, h->stream);
+        h->prof->push_back(r);
+        if (h->prof->size() >= 8192) prof_drain(h);
+    }
+};
 
 inline int check_launch(dnslab *h)
 {
@@ -146,6 +195,7 @@ template <int STAGE> int launch_rk(dnslab *h, double *const *qs, double *const *
     const dim3 blk = tile_block(h);
     const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz / h->zchunk);
     const bool masked = h->face != nullptr, sources = h->nsrc > 0;
+    ProfScope ps(h, DNSLAB_K_RK);
     if (masked && sources) dnsst::k_rk_stage<STAGE, true, true><<<grd, blk, 0, h->stream>>>(a);
     else if (masked) dnsst::k_rk_stage<STAGE, true, false><<<grd, blk, 0, h->stream>>>(a);
     else if (sources) dnsst::k_rk_stage<STAGE, false, true><<<grd, blk, 0, h->stream>>>(a);
@@ -164,6 +214,7 @@ template <int L, int DIR, bool PRO> int launch_fft_x_L(dnslab *h, const c2 *in, 
     size_t nl = 256 / T;
     if (nl > nlines) nl = nlines;
     const size_t smem = nl * (L + L / 8) * sizeof(c2);
+    ProfScope ps(h, DNSLAB_K_FFT_X);
     dnsfft::k_fft_x<L, DIR, PRO><<<(unsigned)(nlines / nl), (unsigned)(nl * T), smem, h->stream>>>(in, out, h->tw[0], (int)nl, ra);
     return check_launch(h);
 }
@@ -201,6 +252,7 @@ template <int L, int XT, int DIR> int launch_fft_col_LX(dnslab *h, c2 *data, int
     const size_t smem = (size_t)XT * L * sizeof(c2);
     auto kern = dnsfft::k_fft_col<L, XT, DIR>;
     if (int rc = set_smem(kern, smem)) return rc;
+    ProfScope ps(h, DNSLAB_K_FFT_Y);
     kern<<<(unsigned)((mx / XT) * nother), XT * T, smem, h->stream>>>(data, h->tw[axis], mx, stride, other_stride);
     return check_launch(h);
 }
@@ -234,6 +286,7 @@ template <int L, int XT> int launch_fft_z_solve_LX(dnslab *h, c2 *data)
     const size_t smem = (size_t)XT * L * sizeof(c2);
     auto kern = dnsfft::k_fft_z_solve<L, XT>;
     if (int rc = set_smem(kern, smem)) return rc;
+    ProfScope ps(h, DNSLAB_K_FFT_Z);
     const double inv_n = 2.0 / (double)h->n; // the packed transform has n/2 complex points
     kern<<<(unsigned)((mx / XT) * h->P.ny), XT * T, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], inv_n);
     return check_launch(h);
@@ -284,6 +337,7 @@ int launch_div(dnslab *h, double *const *q)
 {
     const dim3 blk = tile_block(h);
     const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz);
+    ProfScope ps(h, DNSLAB_K_DIV);
     dnsst::k_div<<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], h->d, h->P.nx, h->P.ny, h->P.nz, 1.0 / (2.0 * h->P.dx),
                                               1.0 / (2.0 * h->P.dy), 1.0 / (2.0 * h->P.dz));
     return check_launch(h);
@@ -294,6 +348,7 @@ int launch_project(dnslab *h, double *const *q, const double *p)
     const dim3 blk = tile_block(h);
     const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz);
     const double r2x = 1.0 / (2.0 * h->P.dx), r2y = 1.0 / (2.0 * h->P.dy), r2z = 1.0 / (2.0 * h->P.dz);
+    ProfScope ps(h, DNSLAB_K_PROJECT);
     if (h->face) dnsst::k_project<true><<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], p, h->face, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
     else dnsst::k_project<false><<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], p, nullptr, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
     return check_launch(h);
@@ -522,9 +577,38 @@ int dnslab_get_fields(dnslab_t *h, double *u, double *v, double *w, double *c, d
 
 int64_t dnslab_launch_count(const dnslab_t *h) { return h ? h->launches : -1; }
 
+int dnslab_profile(dnslab_t *h, int enable)
+{
+    if (!h) return DNSLAB_EINVAL;
+    if (int rc = prof_drain(h)) return rc;
+    if (enable && !h->prof) h->prof = new (std::nothrow) std::vector<ProfRec>();
+    if (enable && !h->prof) return DNSLAB_ENOMEM;
+    if (enable) {
+        for (int c = 0; c < DNSLAB_NCLASS; ++c) {
+            h->prof_ms[c] = 0.0;
+            h->prof_n[c] = 0;
+        }
+    }
+    h->prof_on = enable != 0;
+    return DNSLAB_OK;
+}
+
+int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches)
+{
+    if (!h || !ms || !launches) return DNSLAB_EINVAL;
+    if (int rc = prof_drain(h)) return rc;
+    for (int c = 0; c < DNSLAB_NCLASS; ++c) {
+        ms[c] = h->prof_ms[c];
+        launches[c] = h->prof_n[c];
+    }
+    return DNSLAB_OK;
+}
+
 int dnslab_destroy(dnslab_t *h)
 {
     if (!h) return DNSLAB_EINVAL;
+    prof_drain(h);
+    delete h->prof;
     delete h;
     return DNSLAB_OK;
 }
