@@ -98,7 +98,7 @@ struct dnslab {
     int nsrc;
     dnsst::SourceDev src[DNSLAB_MAX_SOURCES];
     int64_t launches;
-    int zchunk;
+    dim3 rk_block;
     // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
     bool prof_on;
     std::vector<ProfRec> *prof;
@@ -168,7 +168,8 @@ dim3 tile_block(const dnslab *h)
 }
 
 // ---- RK stage ---------------------------------------------------------------------------
-template <int STAGE> int launch_rk(dnslab *h, double *const *qs, double *const *qo)
+// qs: stage field (stencil input); qo: next stage field; elim: Qc eliminated
+template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, double *const *qo, double *const *q2, double *const *q3)
 {
     static const double ca[4] = {0.5, 0.5, 1.0, 0.0};
     static const double cb[4] = {1.0 / 6.0, 1.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0};
@@ -177,12 +178,13 @@ template <int STAGE> int launch_rk(dnslab *h, double *const *qs, double *const *
     for (int m = 0; m < 4; ++m) {
         a.qs[m] = qs[m];
         a.qn[m] = h->Q[m];
-        a.qc[m] = h->Qc[m];
+        a.qc[m] = ELIM ? (q2 ? q2[m] : nullptr) : h->Qc[m];
+        a.q3[m] = q3 ? q3[m] : nullptr;
         a.qo[m] = qo ? qo[m] : nullptr;
-        a.qco[m] = h->Qc[m];
+        a.qco[m] = ELIM ? (q2 ? q2[m] : nullptr) : h->Qc[m];
     }
     a.face = h->face;
-    a.nx = h->P.nx; a.ny = h->P.ny; a.nz = h->P.nz; a.zchunk = h->zchunk;
+    a.nx = h->P.nx; a.ny = h->P.ny; a.nz = h->P.nz;
     a.r2x = 1.0 / (2.0 * h->P.dx); a.r2y = 1.0 / (2.0 * h->P.dy); a.r2z = 1.0 / (2.0 * h->P.dz);
     a.rxx = 1.0 / (h->P.dx * h->P.dx); a.ryy = 1.0 / (h->P.dy * h->P.dy); a.rzz = 1.0 / (h->P.dz * h->P.dz);
     a.nu = h->P.nu; a.ac = h->P.alpha_c;
@@ -192,14 +194,14 @@ template <int STAGE> int launch_rk(dnslab *h, double *const *qs, double *const *
     a.nsrc = h->nsrc;
     a.stab = h->stab;
     for (int s = 0; s < h->nsrc; ++s) a.src[s] = h->src[s];
-    const dim3 blk = tile_block(h);
-    const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz / h->zchunk);
+    const dim3 blk = h->rk_block;
+    const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz / blk.z);
     const bool masked = h->face != nullptr, sources = h->nsrc > 0;
     ProfScope ps(h, DNSLAB_K_RK);
-    if (masked && sources) dnsst::k_rk_stage<STAGE, true, true><<<grd, blk, 0, h->stream>>>(a);
-    else if (masked) dnsst::k_rk_stage<STAGE, true, false><<<grd, blk, 0, h->stream>>>(a);
-    else if (sources) dnsst::k_rk_stage<STAGE, false, true><<<grd, blk, 0, h->stream>>>(a);
-    else dnsst::k_rk_stage<STAGE, false, false><<<grd, blk, 0, h->stream>>>(a);
+    if (masked && sources) dnsst::k_rk<STAGE, ELIM, true, true><<<grd, blk, 0, h->stream>>>(a);
+    else if (masked) dnsst::k_rk<STAGE, ELIM, true, false><<<grd, blk, 0, h->stream>>>(a);
+    else if (sources) dnsst::k_rk<STAGE, ELIM, false, true><<<grd, blk, 0, h->stream>>>(a);
+    else dnsst::k_rk<STAGE, ELIM, false, false><<<grd, blk, 0, h->stream>>>(a);
     return check_launch(h);
 }
 
@@ -418,7 +420,14 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
     h->d = fld(17);
     h->W = fld(18);
     h->ps = (params->flags & 2u) ? fld(19) : nullptr;
-    h->zchunk = params->nz < 16 ? params->nz : 16;
+    {
+        // 64 x 2 x 2 brick (256 threads); narrower in x on tiny grids
+        unsigned bx = params->nx < 64 ? params->nx : 64, by = 2, bz = 2;
+        if (const char *v = getenv("DNSLAB_RK_BLOCK")) sscanf(v, "%u,%u,%u", &bx, &by, &bz);
+        while (bx * by * bz < 256 && by < (unsigned)params->ny && by <= bz) by *= 2;
+        while (bx * by * bz < 256 && bz < (unsigned)params->nz) bz *= 2;
+        h->rk_block = dim3(bx, by, bz);
+    }
 
     auto fail = [&](int rc) { delete h; return rc; };
 #define CKF(call) do { if ((call) != cudaSuccess) return fail(DNSLAB_ECUDA); } while (0)
@@ -522,22 +531,31 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
     const size_t bytes = h->n * sizeof(double);
     int rc;
     for (int it = 0; it < nsteps; ++it) {
-        if ((rc = launch_rk<1>(h, h->Q, h->A))) return rc;
-        if (stage_proj) {
-            CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
-            if ((rc = pressure_stage(h, h->A, h->ps))) return rc;
+        if (!stage_proj) {
+            // Qc eliminated: A = Q2 (then Q*), Bf = Q3, Qc = Q4
+            if ((rc = launch_rk<1, true>(h, h->Q, h->A, nullptr, nullptr))) return rc;
+            if ((rc = launch_rk<2, true>(h, h->A, h->Bf, nullptr, nullptr))) return rc;
+            if ((rc = launch_rk<3, true>(h, h->Bf, h->Qc, nullptr, nullptr))) return rc;
+            if ((rc = launch_rk<4, true>(h, h->Qc, nullptr, h->A, h->Bf))) return rc;
+            if ((rc = pressure_stage(h, h->A, h->p))) return rc;
+            for (int m = 0; m < 4; ++m) {
+                double *t = h->Q[m];
+                h->Q[m] = h->A[m];
+                h->A[m] = t;
+            }
+            continue;
         }
-        if ((rc = launch_rk<2>(h, h->A, h->Bf))) return rc;
-        if (stage_proj) {
-            CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
-            if ((rc = pressure_stage(h, h->Bf, h->ps))) return rc;
-        }
-        if ((rc = launch_rk<3>(h, h->Bf, h->A))) return rc;
-        if (stage_proj) {
-            CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
-            if ((rc = pressure_stage(h, h->A, h->ps))) return rc;
-        }
-        if ((rc = launch_rk<4>(h, h->A, nullptr))) return rc;
+        // NEXT-2 variant: every stage field is projected, so the accumulate form is needed
+        if ((rc = launch_rk<1, false>(h, h->Q, h->A, nullptr, nullptr))) return rc;
+        CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
+        if ((rc = pressure_stage(h, h->A, h->ps))) return rc;
+        if ((rc = launch_rk<2, false>(h, h->A, h->Bf, nullptr, nullptr))) return rc;
+        CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
+        if ((rc = pressure_stage(h, h->Bf, h->ps))) return rc;
+        if ((rc = launch_rk<3, false>(h, h->Bf, h->A, nullptr, nullptr))) return rc;
+        CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
+        if ((rc = pressure_stage(h, h->A, h->ps))) return rc;
+        if ((rc = launch_rk<4, false>(h, h->A, nullptr, nullptr, nullptr))) return rc;
         if ((rc = pressure_stage(h, h->Qc, h->p))) return rc;
         for (int m = 0; m < 4; ++m) {
             double *t = h->Q[m];

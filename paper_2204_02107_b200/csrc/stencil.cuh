@@ -47,11 +47,12 @@ struct SourceDev {
 struct RKArgs {
     const double *qs[4]; // stage field (stencil input)
     const double *qn[4]; // Q^n
-    const double *qc[4]; // running combination, read (stages 2-4)
+    const double *qc[4]; // running combination Qc, read (stages 2-4); with ELIM at stage 4: Q2
+    const double *q3[4]; // ELIM, stage 4 only: Q3
     double *qo[4];       // next stage field, written (stages 1-3)
-    double *qco[4];      // running combination, written
+    double *qco[4];      // Qc written (accumulate form); with ELIM at stage 4: Q* (aliases Q2)
     const uint8_t *face; // null: no solid cells
-    int nx, ny, nz, zchunk;
+    int nx, ny, nz;
     double r2x, r2y, r2z;    // 1/(2 D_a)
     double rxx, ryy, rzz;    // 1/D_a^2
     double nu, ac;           // viscosity, scalar diffusivity
@@ -62,101 +63,103 @@ struct RKArgs {
     SourceDev src[DNS_MAX_SRC];
 };
 
-// One RK stage (a1-a3 of DESIGN.md): F = beta ? RHS(Qs) : 0; Qc(+)= b_s dt F; Qs' = Qn + a_s dt F.
-// Block = 32 x by 8 y cells (narrower in x on tiny grids); each thread marches zchunk planes in z keeping the k-1, k, k+1
-// values of the four fields in registers; x and y neighbours come through L1.
-//   STAGE 1: Qs == Qn, Qc is written fresh (= Qn + b dt F).   STAGE 4: no next stage field.
-template <int STAGE, bool MASKED, bool SOURCES> __global__ void __launch_bounds__(256) k_rk_stage(const RKArgs a)
+// One RK stage (a1-a3 of DESIGN.md): F = beta ? RHS(Qs) : +0.0 fused with the stage update.
+// One thread per cell; a block is a small 3-D brick so that x, y and z neighbours are shared
+// through L1 (DRAM traffic stays at the compulsory bytes, see profiles/).
+//
+// ELIM = false, the accumulate form of the oracle:   Qc (+)= b_s dt F ;  Qs' = Qn + a_s dt F.
+// ELIM = true, Qc eliminated algebraically (12 fewer field passes per step):
+//     stages 1-3:  Qs' = Qn + a_s dt F
+//     stage 4:     Q*  = (-Qn + Q2 + 2 Q3 + Q4)/3 + (dt/6) F4
+//   which equals Qn + dt/6 (F1 + 2 F2 + 2 F3 + F4) because Q2 = Qn + dt/2 F1, Q3 = Qn + dt/2 F2,
+//   Q4 = Qn + dt F3 (classical RK4).  Q* overwrites Q2 in place.
+template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __launch_bounds__(256, 3) k_rk(const RKArgs a)
 {
     const int nx = a.nx, ny = a.ny, nz = a.nz;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k0 = blockIdx.z * a.zchunk;
+    const int k = blockIdx.z * blockDim.z + threadIdx.z;
     const int ip = (i + 1) & (nx - 1), im = (i - 1) & (nx - 1);
-    const int jp = (j + 1) & (ny - 1), jm = (j - 1) & (ny - 1);
     const size_t plane = (size_t)nx * ny;
-    const size_t rowc = (size_t)nx * j, rowp = (size_t)nx * jp, rowm = (size_t)nx * jm;
-
-    double fm[4], f0[4], fp[4];
-    {
-        const size_t om = plane * ((k0 - 1) & (nz - 1)) + rowc + i;
-        const size_t oc = plane * k0 + rowc + i;
+    const size_t pk = plane * k, rowc = (size_t)nx * j;
+    const size_t o = pk + rowc + i;
+    const size_t oyp = pk + (size_t)nx * ((j + 1) & (ny - 1)) + i, oym = pk + (size_t)nx * ((j - 1) & (ny - 1)) + i;
+    const size_t ozp = plane * ((k + 1) & (nz - 1)) + rowc + i, ozm = plane * ((k - 1) & (nz - 1)) + rowc + i;
+    unsigned f = 0x7f;
+    if (MASKED) f = a.face[o];
+    double f0[4], xp[4], xm[4], yp[4], ym[4], fp[4], fm[4], qn[4], qc[4], q3[4];
 #pragma unroll
-        for (int m = 0; m < 4; ++m) {
-            fm[m] = __ldg(&a.qs[m][om]);
-            f0[m] = __ldg(&a.qs[m][oc]);
+    for (int m = 0; m < 4; ++m) {
+        f0[m] = __ldg(&a.qs[m][o]);
+        xp[m] = __ldg(&a.qs[m][pk + rowc + ip]);
+        xm[m] = __ldg(&a.qs[m][pk + rowc + im]);
+        yp[m] = __ldg(&a.qs[m][oyp]);
+        ym[m] = __ldg(&a.qs[m][oym]);
+        fp[m] = __ldg(&a.qs[m][ozp]);
+        fm[m] = __ldg(&a.qs[m][ozm]);
+        qn[m] = f0[m];
+        if (STAGE >= 2 && (STAGE <= 3 || ELIM)) qn[m] = __ldg(&a.qn[m][o]);
+        qc[m] = qn[m];
+        if (STAGE >= 2 && !ELIM) qc[m] = a.qc[m][o]; // plain loads: updated in place
+        if (STAGE == 4 && ELIM) {
+            qc[m] = a.qc[m][o]; // Q2, overwritten below by Q*
+            q3[m] = __ldg(&a.q3[m][o]);
         }
     }
-    for (int kk = 0; kk < a.zchunk; ++kk) {
-        const int k = k0 + kk;
-        const size_t pk = plane * k;
-        const size_t pkp = plane * ((k + 1) & (nz - 1));
-        const size_t o = pk + rowc + i;
-        double xp[4], xm[4], yp[4], ym[4];
+    double F[4];
+    if (!MASKED || (f & 1)) {
+        const double u = f0[0], v = f0[1], w = f0[2];
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            fp[m] = __ldg(&a.qs[m][pkp + rowc + i]);
-            xp[m] = __ldg(&a.qs[m][pk + rowc + ip]);
-            xm[m] = __ldg(&a.qs[m][pk + rowc + im]);
-            yp[m] = __ldg(&a.qs[m][pk + rowp + i]);
-            ym[m] = __ldg(&a.qs[m][pk + rowm + i]);
-        }
-        unsigned f = 0x7f;
-        if (MASKED) f = a.face[o];
-        double F[4];
-        if (!MASKED || (f & 1)) {
-            const double u = f0[0], v = f0[1], w = f0[2];
-#pragma unroll
-            for (int m = 0; m < 4; ++m) {
-                const double c0 = f0[m];
-                double conv = 0.0;
-                conv += (xp[0] * xp[m] - xm[0] * xm[m]) * a.r2x + u * (xp[m] - xm[m]) * a.r2x;
-                conv += (yp[1] * yp[m] - ym[1] * ym[m]) * a.r2y + v * (yp[m] - ym[m]) * a.r2y;
-                conv += (fp[2] * fp[m] - fm[2] * fm[m]) * a.r2z + w * (fp[m] - fm[m]) * a.r2z;
-                double diff;
-                if (m < 3 || !MASKED) {
-                    diff = (m < 3 ? a.nu : a.ac) * ((xp[m] - 2.0 * c0 + xm[m]) * a.rxx + (yp[m] - 2.0 * c0 + ym[m]) * a.ryy +
-                                                    (fp[m] - 2.0 * c0 + fm[m]) * a.rzz);
-                } else {
-                    // eq. 4: no flux through solid faces (beta+- = beta * beta[+-1])
-                    const double dxp = (f & 2) ? (xp[m] - c0) : 0.0, dxm = (f & 4) ? (c0 - xm[m]) : 0.0;
-                    const double dyp = (f & 8) ? (yp[m] - c0) : 0.0, dym = (f & 16) ? (c0 - ym[m]) : 0.0;
-                    const double dzp = (f & 32) ? (fp[m] - c0) : 0.0, dzm = (f & 64) ? (c0 - fm[m]) : 0.0;
-                    diff = a.ac * ((dxp - dxm) * a.rxx + (dyp - dym) * a.ryy + (dzp - dzm) * a.rzz);
-                }
-                double val = -0.5 * conv + diff;
-                if (m < 3) val += a.body[m];
-                F[m] = val;
+            const double c0 = f0[m];
+            double conv = 0.0;
+            conv += (xp[0] * xp[m] - xm[0] * xm[m]) * a.r2x + u * (xp[m] - xm[m]) * a.r2x;
+            conv += (yp[1] * yp[m] - ym[1] * ym[m]) * a.r2y + v * (yp[m] - ym[m]) * a.r2y;
+            conv += (fp[2] * fp[m] - fm[2] * fm[m]) * a.r2z + w * (fp[m] - fm[m]) * a.r2z;
+            double diff;
+            if (m < 3 || !MASKED) {
+                diff = (m < 3 ? a.nu : a.ac) * ((xp[m] - 2.0 * c0 + xm[m]) * a.rxx + (yp[m] - 2.0 * c0 + ym[m]) * a.ryy +
+                                                (fp[m] - 2.0 * c0 + fm[m]) * a.rzz);
+            } else {
+                // eq. 4: no flux through solid faces (beta+- = beta * beta[+-1])
+                const double dxp = (f & 2) ? (xp[m] - c0) : 0.0, dxm = (f & 4) ? (c0 - xm[m]) : 0.0;
+                const double dyp = (f & 8) ? (yp[m] - c0) : 0.0, dym = (f & 16) ? (c0 - ym[m]) : 0.0;
+                const double dzp = (f & 32) ? (fp[m] - c0) : 0.0, dzm = (f & 64) ? (c0 - fm[m]) : 0.0;
+                diff = a.ac * ((dxp - dxm) * a.rxx + (dyp - dym) * a.ryy + (dzp - dzm) * a.rzz);
             }
-            if (SOURCES) {
-                for (int s = 0; s < a.nsrc; ++s) {
-                    const double *t = a.stab + a.src[s].off;
-                    const double sy = __ldg(&t[nx + j]), sz = __ldg(&t[nx + ny + k]);
-                    if (sy == 0.0 || sz == 0.0) continue;
-                    const double Sv = __ldg(&t[i]) * sy * sz;
-                    if (Sv == 0.0) continue;
-                    const uint32_t comps = a.src[s].comps;
+            double val = -0.5 * conv + diff;
+            if (m < 3) val += a.body[m];
+            F[m] = val;
+        }
+        if (SOURCES) {
+            for (int s = 0; s < a.nsrc; ++s) {
+                const double *t = a.stab + a.src[s].off;
+                const double sy = __ldg(&t[nx + j]), sz = __ldg(&t[nx + ny + k]);
+                if (sy == 0.0 || sz == 0.0) continue;
+                const double Sv = __ldg(&t[i]) * sy * sz;
+                if (Sv == 0.0) continue;
+                const uint32_t comps = a.src[s].comps;
 #pragma unroll
-                    for (int m = 0; m < 4; ++m)
-                        if (comps & (1u << m)) F[m] += Sv * (a.src[s].set[m] - f0[m]) * a.src[s].rtau;
-                }
+                for (int m = 0; m < 4; ++m)
+                    if (comps & (1u << m)) F[m] += Sv * (a.src[s].set[m] - f0[m]) * a.src[s].rtau;
             }
-        } else {
-#pragma unroll
-            for (int m = 0; m < 4; ++m) F[m] = 0.0;
         }
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            double qn = f0[m];
-            if (STAGE == 2 || STAGE == 3) qn = __ldg(&a.qn[m][o]);
-            const double qc = (STAGE == 1) ? qn : a.qc[m][o]; // plain load: Qc is updated in place
-            a.qco[m][o] = qc + a.cb * F[m];
-            if (STAGE < 4) a.qo[m][o] = qn + a.ca * F[m];
+            if (ELIM) {
+                if (STAGE < 4) a.qo[m][o] = qn[m] + a.ca * F[m];
+                else a.qco[m][o] = (qc[m] - qn[m] + 2.0 * q3[m] + f0[m]) * (1.0 / 3.0) + a.cb * F[m];
+            } else {
+                a.qco[m][o] = qc[m] + a.cb * F[m];
+                if (STAGE < 4) a.qo[m][o] = qn[m] + a.ca * F[m];
+            }
         }
+    } else {
+        // solid cell: every field it holds is +0.0 and stays +0.0 (select)
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            fm[m] = f0[m];
-            f0[m] = fp[m];
+            if (!ELIM || STAGE == 4) a.qco[m][o] = 0.0;
+            if (STAGE < 4) a.qo[m][o] = 0.0;
         }
     }
 }
