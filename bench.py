@@ -93,6 +93,19 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def job_value(ms_local, n_cells, steps, world, device):
+    """Whole-job cell-updates/s of `world` independent replicas: every rank advanced n_cells cells by
+    `steps` steps; the job time is the MAX over ranks of the device-timed milliseconds (no data-path
+    collective: DESIGN.md "replicas only").  Returns (value, ms_max)."""
+    import torch
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    return world * n_cells * steps / (ms_max * 1e-3), ms_max
+
+
 def make_case(cfg, piter):
     from paper_2204_02107_b200 import cases
     case = cases.config(cfg)
@@ -186,11 +199,7 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     launches = s.launch_count() - l0
     clocks = sampler.stop(t0, t1) if sampler else None
-    tms = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    ms_max = float(tms.item())
-    value = world * N * K / (ms_max * 1e-3)
+    value, ms_max = job_value(ms, N, K, world, dev)
 
     # ---- per-kernel pass (same workload, K steps, events around every launch)
     s.profile(True)
@@ -234,10 +243,7 @@ def run_ours(args):
             s.get_fields(**host_out)
         e1.record(s.stream)
         barrier()
-        tms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        e2e_value = world * N * Ke / (float(tms.item()) * 1e-3)
+        e2e_value, _ = job_value(e0.elapsed_time(e1), N, Ke, world, dev)
         assert bool(torch.isfinite(host_out["u"]).all())
 
     out = None
