@@ -33,17 +33,39 @@ def canonical_bytes_per_cell(P, masked):
     return 8.0 * (72 + 10 * P)
 
 
-# algorithmic bytes per cell per launch of each kernel class
-def class_bytes_per_cell(masked):
+# Bytes per cell per launch of each kernel class.
+# "canonical": SURVEY.md 8(d)'s model (accumulate-form RK with Qc: 12+20+20+12 passes; div R3 W1; 5 FFT passes of
+# R1 W1 per solve; dense p^k + mask read per eq. 9 iteration; projection R4 W3).
+# "moved": what this implementation must move (Qc eliminated: 8+12+12+20 passes; eq. 9 only at the near-solid
+# cells, a fraction fb of the grid: index 4 + saved d 8 + d 8 + p centre 8 + face 1 + ~1 neighbour 8 bytes).
+def class_bytes_per_cell(masked, fb=0.0):
     m = 0.125 if masked else 0.0
-    return {
-        "rk_stage": (96 + 160 + 160 + 96) / 4.0 + m,  # stage 1: R4 W8; 2,3: R12 W8; 4: R8 W4
-        "div": 32.0,                                   # R3 W1
-        "fft_x": 16.0 + (8.0 + m) / 2.0,               # R1 W1; the forward pass also reads p^k + mask
+    canonical = {
+        "rk_stage": (96 + 160 + 160 + 96) / 4.0 + m,
+        "div": 32.0,
+        "fft_x": 16.0,
         "fft_y": 16.0,
         "fft_z_solve": 16.0,
-        "project": 56.0 + m,                           # R4 W3
+        "project": 56.0 + m,
+        "eq9_sparse": 8.0 + m,
     }
+    moved = dict(canonical)
+    moved["rk_stage"] = (64 + 96 + 96 + 160) / 4.0 + (1.0 if masked else 0.0)
+    moved["project"] = 56.0 + (1.0 if masked else 0.0)
+    moved["eq9_sparse"] = 37.0 * fb
+    return canonical, moved
+
+
+def near_solid_fraction(mask):
+    """Fraction of cells with at least one solid face neighbour (where eq. 9's bracket can be non-zero)."""
+    import numpy as np
+    if mask is None:
+        return 0.0
+    fluid = mask != 0
+    allf = np.ones(mask.shape, dtype=bool)
+    for ax in range(3):
+        allf &= np.roll(fluid, 1, axis=ax) & np.roll(fluid, -1, axis=ax)
+    return float(1.0 - allf.mean())
 
 
 def load_peak():
@@ -206,21 +228,25 @@ def run_ours(args):
     s.step(K)
     prof = s.profile_read()
     s.profile(False)
-    cb = class_bytes_per_cell(masked)
+    fb = near_solid_fraction(case["mask"])
+    cb, mv = class_bytes_per_cell(masked, fb)
+    prof = {k: v for k, v in prof.items() if v[1] > 0}
     tot_ms = sum(v[0] for v in prof.values()) or 1.0
     dom = max(prof, key=lambda k: prof[k][0])
     d_ms, d_n = prof[dom]
     peak, peak_src = load_peak()
     achieved = cb[dom] * N / (d_ms / d_n * 1e-3) / 1e9
+    achieved_moved = mv[dom] * N / (d_ms / d_n * 1e-3) / 1e9
     breakdown = {k: {"ms_per_step": v[0] / K, "launches_per_step": v[1] / K,
-                     "GBps": (cb[k] * N / (v[0] / v[1] * 1e-3) / 1e9) if v[1] else None} for k, v in prof.items()}
+                     "GBps_canonical": cb[k] * N / (v[0] / v[1] * 1e-3) / 1e9,
+                     "GBps_moved": mv[k] * N / (v[0] / v[1] * 1e-3) / 1e9} for k, v in prof.items()}
     traffic = None
-    tfile = os.path.join(ROOT, "profiles", "traffic.json")
+    tfile = os.path.join(ROOT, "profiles", "traffic.csv")   # class,case,dram bytes per launch (ncu --set full)
     if os.path.exists(tfile):
-        try:
-            traffic = json.load(open(tfile)).get(dom, {}).get(case["name"])
-        except Exception:
-            traffic = None
+        for line in open(tfile):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 3 and f[0] == dom and f[1] == case["name"]:
+                traffic = float(f[2])
     step_bytes = canonical_bytes_per_cell(P, masked) * N
     step_gbs = step_bytes / (ms_max / K * 1e-3) / 1e9
 
@@ -265,6 +291,8 @@ def run_ours(args):
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                          "bytes_per_cell_per_launch": cb[dom], "share_of_step": d_ms / tot_ms,
+                         "moved_bytes_per_cell_per_launch": mv[dom], "achieved_moved": achieved_moved,
+                         "frac_moved": achieved_moved / peak, "near_solid_fraction": fb,
                          "timing": "CUDA events around every launch (dnslab_profile), separate pass of K steps"},
             "step_roofline": {"canonical_bytes_per_cell": canonical_bytes_per_cell(P, masked), "achieved": step_gbs,
                               "peak": peak, "unit": "GB/s", "frac": step_gbs / peak},

@@ -55,7 +55,10 @@ typedef struct {
     double dt;             /* fixed time step > 0                                                    */
     double body[3];        /* body force b (eq. 2)                                      */
     int32_t n_piter;       /* eq. 9 iterations >= 1; the paper hard-codes 4           */
-    uint32_t flags;        /* bit0 reserved (eq. 6 filter, not built); bit1: project every RK stage  */
+    uint32_t flags;        /* bit0 reserved (eq. 6 filter, not built); bit1: project every RK stage;
+                              bit2: evaluate eq. 9's right-hand side densely inside the forward x pass
+                              instead of at the listed near-solid cells (same result; the library does
+                              this by itself when more than half of the cells are near-solid)         */
 } dnslab_params_t;
 
 /* One inflow/outflow forcing region S(x,y,z) of eqs. 2-3. */
@@ -118,7 +121,8 @@ int64_t dnslab_launch_count(const dnslab_t *h);
 #define DNSLAB_K_FFT_Y 3   /* y-axis FFT passes                                            */
 #define DNSLAB_K_FFT_Z 4   /* fused z forward + eigenvalue division + z inverse pass       */
 #define DNSLAB_K_PROJECT 5 /* pressure-gradient projection                                 */
-#define DNSLAB_NCLASS 6
+#define DNSLAB_K_EQ9 6     /* eq. 9 right-hand side at the cells next to solid cells       */
+#define DNSLAB_NCLASS 7
 int dnslab_profile(dnslab_t *h, int enable);
 int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches);
 

@@ -28,12 +28,12 @@ bool valid_params(const dnslab_params_t *P)
     if (P->nx < 8 || P->nx > 2048 || P->ny < 8 || P->ny > 1024 || P->nz < 8 || P->nz > 1024) return false;
     if (!(P->dx > 0) || !(P->dy > 0) || !(P->dz > 0) || !(P->dt > 0)) return false;
     if (!(P->nu >= 0) || !(P->alpha_c >= 0) || P->n_piter < 1) return false;
-    if (P->flags & ~2u) return false;
+    if (P->flags & ~6u) return false;
     return true;
 }
 
 struct Layout {
-    size_t field_bytes, off_fields, nfields, off_face, off_tw[3], off_eig, off_stab, total;
+    size_t field_bytes, off_fields, nfields, off_face, off_tw[3], off_eig, off_stab, off_blist, off_bsave, bcap, total;
 };
 
 // 19 fields: Q(4) A(4) B(4) Qc(4) p d W (+1 scratch pressure with per-stage projection)
@@ -57,6 +57,13 @@ Layout make_layout(const dnslab_params_t *P)
     off += align_up((size_t)(P->nx / 2 + P->ny + P->nz) * sizeof(double));
     L.off_stab = off;
     off += align_up((size_t)DNSLAB_MAX_SOURCES * (P->nx + P->ny + P->nz) * sizeof(double));
+    // eq. 9 boundary list (cells with a solid face neighbour) and the compact copy of d there; masks whose
+    // list would be longer than N/2 use the dense prologue of the forward x pass instead
+    L.bcap = n / 2;
+    L.off_blist = off;
+    off += align_up(L.bcap * sizeof(uint32_t));
+    L.off_bsave = off;
+    off += align_up(L.bcap * sizeof(double));
     L.total = off;
     return L;
 }
@@ -92,6 +99,9 @@ struct dnslab {
     Layout L;
     double *Q[4], *A[4], *Bf[4], *Qc[4], *p, *d, *W, *ps;
     uint8_t *face; // null when the mask has no solid cell
+    uint32_t *blist; // eq. 9 boundary list; null: dense prologue in the forward x pass
+    double *bsave;
+    int nb;
     c2 *tw[3];
     double *eig[3];
     double *stab;
@@ -99,6 +109,7 @@ struct dnslab {
     dnsst::SourceDev src[DNSLAB_MAX_SOURCES];
     int64_t launches;
     dim3 rk_block;
+    int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
     // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
     bool prof_on;
     std::vector<ProfRec> *prof;
@@ -194,10 +205,30 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
     a.nsrc = h->nsrc;
     a.stab = h->stab;
     for (int s = 0; s < h->nsrc; ++s) a.src[s] = h->src[s];
-    const dim3 blk = h->rk_block;
-    const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz / blk.z);
     const bool masked = h->face != nullptr, sources = h->nsrc > 0;
     ProfScope ps(h, DNSLAB_K_RK);
+    if (h->rk_kc > 0) {
+        // z-marching kernel: 64 x 8 columns, kc planes per block
+        a.kc = h->rk_kc;
+        const dim3 blk(32, dnsst::RKM_TY, 1);
+        const dim3 grd(h->P.nx / dnsst::RKM_TX, h->P.ny / dnsst::RKM_TY, h->P.nz / h->rk_kc);
+        const size_t smem = dnsst::RKM_SMEM;
+#define DNS_LAUNCH_MARCH(M, S)                                                                                   \
+    do {                                                                                                         \
+        auto kern = dnsst::k_rk_march<STAGE, ELIM, M, S>;                                                        \
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)   \
+            return DNSLAB_ECUDA;                                                                                 \
+        kern<<<grd, blk, smem, h->stream>>>(a);                                                                  \
+    } while (0)
+        if (masked && sources) DNS_LAUNCH_MARCH(true, true);
+        else if (masked) DNS_LAUNCH_MARCH(true, false);
+        else if (sources) DNS_LAUNCH_MARCH(false, true);
+        else DNS_LAUNCH_MARCH(false, false);
+#undef DNS_LAUNCH_MARCH
+        return check_launch(h);
+    }
+    const dim3 blk = h->rk_block;
+    const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz / blk.z);
     if (masked && sources) dnsst::k_rk<STAGE, ELIM, true, true><<<grd, blk, 0, h->stream>>>(a);
     else if (masked) dnsst::k_rk<STAGE, ELIM, true, false><<<grd, blk, 0, h->stream>>>(a);
     else if (sources) dnsst::k_rk<STAGE, ELIM, false, true><<<grd, blk, 0, h->stream>>>(a);
@@ -321,12 +352,13 @@ int launch_fft_z_solve(dnslab *h, c2 *data)
 int poisson_solve(dnslab *h, const double *d, const double *pold, double *pout, bool prologue)
 {
     dnsfft::PoissonRhsArgs ra;
+    prologue = prologue && h->face && !h->blist;
     ra.d = d; ra.p = pold; ra.face = (prologue ? h->face : nullptr);
     ra.nx = h->P.nx; ra.ny = h->P.ny; ra.nz = h->P.nz;
     ra.r2x = 1.0 / (2.0 * h->P.dx); ra.r2y = 1.0 / (2.0 * h->P.dy); ra.r2z = 1.0 / (2.0 * h->P.dz);
     c2 *W = reinterpret_cast<c2 *>(h->W);
     int rc;
-    if (prologue && h->face) rc = launch_fft_x<-1, true>(h, reinterpret_cast<const c2 *>(d), W, ra);
+    if (prologue) rc = launch_fft_x<-1, true>(h, reinterpret_cast<const c2 *>(d), W, ra);
     else rc = launch_fft_x<-1, false>(h, reinterpret_cast<const c2 *>(d), W, ra);
     if (rc) return rc;
     if ((rc = launch_fft_col<-1>(h, W, 1))) return rc;
@@ -356,13 +388,27 @@ int launch_project(dnslab *h, double *const *q, const double *p)
     return check_launch(h);
 }
 
+int launch_eq9_sparse(dnslab *h, const double *p, bool first)
+{
+    int lgx = 0, lgy = 0;
+    while ((1 << lgx) < h->P.nx) ++lgx;
+    while ((1 << lgy) < h->P.ny) ++lgy;
+    ProfScope ps(h, DNSLAB_K_EQ9);
+    dnsst::k_eq9_sparse<<<(unsigned)((h->nb + 255) / 256), 256, 0, h->stream>>>(h->d, p, h->face, h->blist, h->bsave, h->nb, first ? 1 : 0, h->P.nx,
+                                                                              h->P.ny, h->P.nz, lgx, lgy, 1.0 / (2.0 * h->P.dx),
+                                                                              1.0 / (2.0 * h->P.dy), 1.0 / (2.0 * h->P.dz));
+    return check_launch(h);
+}
+
 // divergence, n_piter iterations of eq. 9 warm-started from p, correction (in place on q)
 int pressure_stage(dnslab *h, double *const *q, double *p)
 {
     int rc;
     if ((rc = launch_div(h, q))) return rc;
-    for (int it = 0; it < h->P.n_piter; ++it)
+    for (int it = 0; it < h->P.n_piter; ++it) {
+        if (h->blist && h->nb > 0 && (rc = launch_eq9_sparse(h, p, it == 0))) return rc;
         if ((rc = poisson_solve(h, h->d, p, p, true))) return rc;
+    }
     return launch_project(h, q, p);
 }
 
@@ -427,6 +473,18 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
         while (bx * by * bz < 256 && by < (unsigned)params->ny && by <= bz) by *= 2;
         while (bx * by * bz < 256 && bz < (unsigned)params->nz) bz *= 2;
         h->rk_block = dim3(bx, by, bz);
+        // marching kernel for nx >= 64: enough blocks for >= 6 waves of 2 blocks per SM, at least 8 planes each
+        h->rk_kc = 0;
+        if (params->nx >= dnsst::RKM_TX && !getenv("DNSLAB_RK_BRICK")) {
+            const long tiles = (long)(params->nx / dnsst::RKM_TX) * (params->ny / dnsst::RKM_TY);
+            int kc = params->nz;
+            while (kc > 8 && tiles * (params->nz / kc) < 6L * 2 * prop.multiProcessorCount) kc /= 2;
+            if (const char *v = getenv("DNSLAB_RK_KC")) {
+                const int e = atoi(v);
+                if (e >= 1 && e <= params->nz && params->nz % e == 0) kc = e;
+            }
+            h->rk_kc = kc;
+        }
     }
 
     auto fail = [&](int rc) { delete h; return rc; };
@@ -452,6 +510,33 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
             if (!hm[o]) { any_solid = true; break; }
         if (any_solid) h->face = face;
         CKF(cudaMemsetAsync(h->W, 0, L.field_bytes, h->stream));
+        if (any_solid && !(params->flags & 4u)) {
+            // cells with at least one solid face neighbour, ascending index order
+            const int nx = params->nx, ny = params->ny, nz = params->nz;
+            std::vector<uint32_t> bl;
+            bool fits = true;
+            for (int k = 0; k < nz && fits; ++k) {
+                const size_t kp = (size_t)((k + 1) & (nz - 1)), km = (size_t)((k - 1) & (nz - 1));
+                for (int j = 0; j < ny && fits; ++j) {
+                    const size_t jp = (size_t)((j + 1) & (ny - 1)), jm = (size_t)((j - 1) & (ny - 1));
+                    const uint8_t *r0 = hm.data() + (size_t)nx * (j + (size_t)ny * k);
+                    const uint8_t *ryp = hm.data() + (size_t)nx * (jp + (size_t)ny * k), *rym = hm.data() + (size_t)nx * (jm + (size_t)ny * k);
+                    const uint8_t *rzp = hm.data() + (size_t)nx * (j + (size_t)ny * kp), *rzm = hm.data() + (size_t)nx * (j + (size_t)ny * km);
+                    for (int i = 0; i < nx; ++i) {
+                        if (r0[(i + 1) & (nx - 1)] && r0[(i - 1) & (nx - 1)] && ryp[i] && rym[i] && rzp[i] && rzm[i]) continue;
+                        if (bl.size() >= L.bcap) { fits = false; break; }
+                        bl.push_back((uint32_t)((size_t)i + (size_t)nx * (j + (size_t)ny * k)));
+                    }
+                }
+            }
+            if (fits) {
+                h->blist = (uint32_t *)(h->ws + L.off_blist);
+                h->bsave = (double *)(h->ws + L.off_bsave);
+                h->nb = (int)bl.size();
+                if (h->nb) CKF(cudaMemcpyAsync(h->blist, bl.data(), bl.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, h->stream));
+                CKF(cudaStreamSynchronize(h->stream));
+            }
+        }
     }
 
     // twiddles exp(-2 pi i t/L) per axis and eigenvalue parts (sin(2 pi k/N_a)/D_a)^2

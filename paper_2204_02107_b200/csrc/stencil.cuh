@@ -59,6 +59,7 @@ struct RKArgs {
     double body[3];
     double ca, cb;           // a_s dt, b_s dt
     int nsrc;
+    int kc;                  // k_rk_march: planes per block
     const double *stab;
     SourceDev src[DNS_MAX_SRC];
 };
@@ -164,6 +165,209 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// k_rk_march: the same stage (a1-a3) for grids with nx >= 64, marching along z.
+//
+// A block owns a 64 x 8 (x by y) column of cells and walks kc planes of it.  Each thread owns two
+// x-adjacent cells (one double2 per field).  The stage field's plane k+2 is in flight (cp.async,
+// LDGSTS) into one of three shared-memory plane tiles (4 fields x 10 rows x 64+2 cells, halo included,
+// periodic wrap applied to the source address) while plane k is being computed: x/y neighbours come
+// from the tile of plane k, the z+1 neighbour from the tile of plane k+1, the z-1 neighbour and the
+// centre are carried in registers.  So every stage-field value is fetched from L2/HBM once per block
+// (plus the one-cell halo), the bytes in flight live in shared memory rather than in registers, and
+// the other operands (Qn, Q2, Q3) and the result are streamed as 16-byte accesses.
+// One __syncthreads per plane.  Arithmetic and select semantics are those of k_rk above.
+constexpr int RKM_TX = 64, RKM_TY = 8, RKM_SW = 68, RKM_ROWS = RKM_TY + 2, RKM_NBUF = 3;
+constexpr int RKM_SMEM = RKM_NBUF * 4 * RKM_ROWS * RKM_SW * (int)sizeof(double);
+
+__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void *dst_smem, const void *src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
+
+// RHS of one cell for field m given its seven-point neighbourhood and the advecting velocities.
+template <bool MASKED_C>
+__device__ __forceinline__ double rk_rhs_cell(const RKArgs &a, int m, unsigned f, double c0, double xp, double xm, double yp, double ym,
+                                              double zp, double zm, double u, double v, double w, double uxp, double uxm, double vyp,
+                                              double vym, double wzp, double wzm)
+{
+    double conv = ((uxp * xp - uxm * xm) + u * (xp - xm)) * a.r2x;
+    conv += ((vyp * yp - vym * ym) + v * (yp - ym)) * a.r2y;
+    conv += ((wzp * zp - wzm * zm) + w * (zp - zm)) * a.r2z;
+    double diff;
+    if (!MASKED_C) {
+        diff = (m < 3 ? a.nu : a.ac) * ((xp - 2.0 * c0 + xm) * a.rxx + (yp - 2.0 * c0 + ym) * a.ryy + (zp - 2.0 * c0 + zm) * a.rzz);
+    } else {
+        // eq. 4: no flux through solid faces (beta+- = beta * beta[+-1])
+        const double dxp = (f & 2) ? (xp - c0) : 0.0, dxm = (f & 4) ? (c0 - xm) : 0.0;
+        const double dyp = (f & 8) ? (yp - c0) : 0.0, dym = (f & 16) ? (c0 - ym) : 0.0;
+        const double dzp = (f & 32) ? (zp - c0) : 0.0, dzm = (f & 64) ? (c0 - zm) : 0.0;
+        diff = a.ac * ((dxp - dxm) * a.rxx + (dyp - dym) * a.ryy + (dzp - dzm) * a.rzz);
+    }
+    double val = -0.5 * conv + diff;
+    if (m < 3) val += a.body[m];
+    return val;
+}
+
+template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __launch_bounds__(256, 2) k_rk_march(const RKArgs a)
+{
+    constexpr int TX = RKM_TX, SW = RKM_SW, ROWS = RKM_ROWS, PLANE = 4 * RKM_ROWS * RKM_SW;
+    extern __shared__ double2 rkm_smem2[];
+    double *sm = reinterpret_cast<double *>(rkm_smem2);
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * 32 + tx;
+    const int nx = a.nx, ny = a.ny, nz = a.nz, kc = a.kc;
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * RKM_TY, k0 = blockIdx.z * kc;
+    const int i = x0 + 2 * tx, j = y0 + ty;
+    const size_t plane = (size_t)nx * ny;
+    const size_t orow = (size_t)nx * j + i;
+
+    // this thread's share of one plane tile: per field 10 rows x 32 double2 (interior + y halo) and 20 x-halo values
+    const int r_a = tid >> 5, q_a = tid & 31;                 // copy A: rows 0..7
+    const size_t src_a = (size_t)nx * ((y0 - 1 + r_a) & (ny - 1)) + x0 + 2 * q_a;
+    const int dst_a = r_a * SW + 2 + 2 * q_a;
+    const bool has_b = tid < 64;                              // copy B: rows 8..9
+    const size_t src_b = (size_t)nx * ((y0 + 7 + r_a) & (ny - 1)) + x0 + 2 * q_a;
+    const int dst_b = (8 + r_a) * SW + 2 + 2 * q_a;
+    const bool has_h = tid >= 64 && tid < 64 + 4 * ROWS * 2;  // x halo: 80 values
+    const int hh = tid - 64, h_m = hh / (ROWS * 2), h_r = (hh % (ROWS * 2)) >> 1, h_s = hh & 1;
+    const size_t src_h = (size_t)nx * ((y0 - 1 + h_r) & (ny - 1)) + (h_s ? ((x0 + TX) & (nx - 1)) : ((x0 - 1) & (nx - 1)));
+    const int dst_h = (h_m * ROWS + h_r) * SW + (h_s ? 2 + TX : 1);
+    auto issue_plane = [&](int kk, int buf) {
+        const size_t pk = plane * (size_t)(kk & (nz - 1));
+        double *sb = sm + buf * PLANE;
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            cp_async16(sb + m * ROWS * SW + dst_a, a.qs[m] + pk + src_a);
+            if (has_b) cp_async16(sb + m * ROWS * SW + dst_b, a.qs[m] + pk + src_b);
+        }
+        if (has_h) cp_async8(sb + dst_h, a.qs[h_m] + pk + src_h);
+        cp_async_commit();
+    };
+
+    issue_plane(k0, 0);
+    issue_plane(k0 + 1, 1);
+    double2 zm[4], cur[4];
+    {
+        const size_t pkm = plane * (size_t)((k0 - 1) & (nz - 1));
+#pragma unroll
+        for (int m = 0; m < 4; ++m) zm[m] = __ldg(reinterpret_cast<const double2 *>(a.qs[m] + pkm + orow));
+    }
+    const int own = (ty + 1) * SW + 2 + 2 * tx; // this thread's pair inside a field's tile
+
+    for (int t = 0; t < kc; ++t) {
+        const int k = k0 + t;
+        const size_t o = plane * (size_t)k + orow;
+        // operands that do not go through shared memory: issue their loads before waiting
+        double2 qn[4], q2[4], q3[4];
+        unsigned fA = 0x7f, fB = 0x7f;
+        if (MASKED) {
+            const uchar2 fv = *reinterpret_cast<const uchar2 *>(a.face + o);
+            fA = fv.x;
+            fB = fv.y;
+        }
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            if (STAGE >= 2) qn[m] = __ldg(reinterpret_cast<const double2 *>(a.qn[m] + o));
+            if (STAGE >= 2 && !ELIM) q2[m] = *reinterpret_cast<const double2 *>(a.qc[m] + o); // Qc, updated in place
+            if (STAGE == 4 && ELIM) {
+                q2[m] = *reinterpret_cast<const double2 *>(a.qc[m] + o); // Q2, overwritten below by Q*
+                q3[m] = __ldg(reinterpret_cast<const double2 *>(a.q3[m] + o));
+            }
+        }
+        cp_async_wait_all();
+        __syncthreads(); // plane k+1 visible to all; every thread is done with the tile of plane k-1
+        if (t + 2 <= kc) issue_plane(k + 2, (t + 2) % RKM_NBUF);
+        const double *sC = sm + (t % RKM_NBUF) * PLANE, *sN = sm + ((t + 1) % RKM_NBUF) * PLANE;
+        if (t == 0) {
+#pragma unroll
+            for (int m = 0; m < 4; ++m) cur[m] = *reinterpret_cast<const double2 *>(sC + m * ROWS * SW + own);
+        }
+        double2 zp[4];
+#pragma unroll
+        for (int m = 0; m < 4; ++m) zp[m] = *reinterpret_cast<const double2 *>(sN + m * ROWS * SW + own);
+        if (STAGE == 1) {
+#pragma unroll
+            for (int m = 0; m < 4; ++m) qn[m] = cur[m];
+        }
+        const double2 vym = *reinterpret_cast<const double2 *>(sC + 1 * ROWS * SW + own - SW);
+        const double2 vyp = *reinterpret_cast<const double2 *>(sC + 1 * ROWS * SW + own + SW);
+        const double uxmA = sC[own - 1], uxpB = sC[own + 2];
+        double2 F[4];
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            const double *sf = sC + m * ROWS * SW + own;
+            const double2 ym = *reinterpret_cast<const double2 *>(sf - SW), yp = *reinterpret_cast<const double2 *>(sf + SW);
+            const double xmA = sf[-1], xpB = sf[2];
+            if (m < 3 || !MASKED) {
+                F[m].x = rk_rhs_cell<false>(a, m, fA, cur[m].x, cur[m].y, xmA, yp.x, ym.x, zp[m].x, zm[m].x, cur[0].x, cur[1].x, cur[2].x,
+                                            cur[0].y, uxmA, vyp.x, vym.x, zp[2].x, zm[2].x);
+                F[m].y = rk_rhs_cell<false>(a, m, fB, cur[m].y, xpB, cur[m].x, yp.y, ym.y, zp[m].y, zm[m].y, cur[0].y, cur[1].y, cur[2].y,
+                                            uxpB, cur[0].x, vyp.y, vym.y, zp[2].y, zm[2].y);
+            } else {
+                F[m].x = rk_rhs_cell<true>(a, m, fA, cur[m].x, cur[m].y, xmA, yp.x, ym.x, zp[m].x, zm[m].x, cur[0].x, cur[1].x, cur[2].x,
+                                           cur[0].y, uxmA, vyp.x, vym.x, zp[2].x, zm[2].x);
+                F[m].y = rk_rhs_cell<true>(a, m, fB, cur[m].y, xpB, cur[m].x, yp.y, ym.y, zp[m].y, zm[m].y, cur[0].y, cur[1].y, cur[2].y,
+                                           uxpB, cur[0].x, vyp.y, vym.y, zp[2].y, zm[2].y);
+            }
+        }
+        if (SOURCES) {
+            for (int s = 0; s < a.nsrc; ++s) {
+                const double *tb = a.stab + a.src[s].off;
+                const double sz = __ldg(&tb[nx + ny + k]), sy = __ldg(&tb[nx + j]);
+                if (sy == 0.0 || sz == 0.0) continue;
+                const double2 sx = __ldg(reinterpret_cast<const double2 *>(tb + i));
+                const double SA = sx.x * sy * sz, SB = sx.y * sy * sz;
+                const uint32_t comps = a.src[s].comps;
+#pragma unroll
+                for (int m = 0; m < 4; ++m)
+                    if (comps & (1u << m)) {
+                        if (SA != 0.0) F[m].x += SA * (a.src[s].set[m] - cur[m].x) * a.src[s].rtau;
+                        if (SB != 0.0) F[m].y += SB * (a.src[s].set[m] - cur[m].y) * a.src[s].rtau;
+                    }
+            }
+        }
+        const bool flA = !MASKED || (fA & 1), flB = !MASKED || (fB & 1);
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            // solid cell: every field it holds is +0.0 and stays +0.0 (select)
+            if (ELIM) {
+                double2 r;
+                if (STAGE < 4) {
+                    r.x = flA ? qn[m].x + a.ca * F[m].x : 0.0;
+                    r.y = flB ? qn[m].y + a.ca * F[m].y : 0.0;
+                    *reinterpret_cast<double2 *>(a.qo[m] + o) = r;
+                } else {
+                    r.x = flA ? (q2[m].x - qn[m].x + 2.0 * q3[m].x + cur[m].x) * (1.0 / 3.0) + a.cb * F[m].x : 0.0;
+                    r.y = flB ? (q2[m].y - qn[m].y + 2.0 * q3[m].y + cur[m].y) * (1.0 / 3.0) + a.cb * F[m].y : 0.0;
+                    *reinterpret_cast<double2 *>(a.qco[m] + o) = r;
+                }
+            } else {
+                double2 c, r;
+                const double2 qcv = STAGE >= 2 ? q2[m] : qn[m];
+                c.x = flA ? qcv.x + a.cb * F[m].x : 0.0;
+                c.y = flB ? qcv.y + a.cb * F[m].y : 0.0;
+                *reinterpret_cast<double2 *>(a.qco[m] + o) = c;
+                if (STAGE < 4) {
+                    r.x = flA ? qn[m].x + a.ca * F[m].x : 0.0;
+                    r.y = flB ? qn[m].y + a.ca * F[m].y : 0.0;
+                    *reinterpret_cast<double2 *>(a.qo[m] + o) = r;
+                }
+            }
+        }
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            zm[m] = cur[m];
+            cur[m] = zp[m];
+        }
+    }
+}
+
 // a4: d = sum_a delta_a u_a (eq. 7 right-hand side)
 __global__ void __launch_bounds__(256) k_div(const double *__restrict__ u, const double *__restrict__ v, const double *__restrict__ w,
                                              double *__restrict__ d, int nx, int ny, int nz, double r2x, double r2y, double r2z)
@@ -177,6 +381,40 @@ __global__ void __launch_bounds__(256) k_div(const double *__restrict__ u, const
     d[o] = (__ldg(&u[row + ((i + 1) & (nx - 1))]) - __ldg(&u[row + ((i - 1) & (nx - 1))])) * r2x +
            (__ldg(&v[plane * k + (size_t)nx * ((j + 1) & (ny - 1)) + i]) - __ldg(&v[plane * k + (size_t)nx * ((j - 1) & (ny - 1)) + i])) * r2y +
            (__ldg(&w[plane * ((k + 1) & (nz - 1)) + (size_t)nx * j + i]) - __ldg(&w[plane * ((k - 1) & (nz - 1)) + (size_t)nx * j + i])) * r2z;
+}
+
+// a5, right-hand side of eq. 9: r = d + sum_a delta_a[(1-beta) delta_a p], evaluated only
+// where the bracket can be non-zero.  (1-beta) is 0 in the fluid, so those are the cells with at least
+// one solid face neighbour; `list` holds their linear indices in ascending order (built at create).
+// The first iteration of a step saves d at those cells (`save`), later ones restore it from there, and
+// r overwrites d in place: everywhere else r == d already, so the forward x pass reads one plain array.
+// face: bit0 beta(cell), bit1/2 beta(x+1/x-1), bit3/4 beta(y+1/y-1), bit5/6 beta(z+1/z-1).
+__global__ void __launch_bounds__(256) k_eq9_sparse(double *__restrict__ d, const double *__restrict__ p, const uint8_t *__restrict__ face,
+                                                    const uint32_t *__restrict__ list, double *__restrict__ save, int nlist, int first,
+                                                    int nx, int ny, int nz, int lgx, int lgy, double r2x, double r2y, double r2z)
+{
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= nlist) return;
+    const uint32_t o = list[n];
+    const int i = o & (nx - 1), j = (o >> lgx) & (ny - 1), k = o >> (lgx + lgy);
+    const unsigned f = face[o];
+    double dv;
+    if (first) {
+        dv = d[o];
+        save[n] = dv;
+    } else {
+        dv = save[n];
+    }
+    const size_t row = (size_t)nx * ((size_t)j + (size_t)ny * k);
+    const double pc = __ldg(&p[o]);
+    double gxp = 0.0, gxm = 0.0, gyp = 0.0, gym = 0.0, gzp = 0.0, gzm = 0.0;
+    if (!(f & 2)) gxp = (__ldg(&p[row + ((i + 2) & (nx - 1))]) - pc) * r2x;
+    if (!(f & 4)) gxm = (pc - __ldg(&p[row + ((i - 2) & (nx - 1))])) * r2x;
+    if (!(f & 8)) gyp = (__ldg(&p[(size_t)nx * ((size_t)((j + 2) & (ny - 1)) + (size_t)ny * k) + i]) - pc) * r2y;
+    if (!(f & 16)) gym = (pc - __ldg(&p[(size_t)nx * ((size_t)((j - 2) & (ny - 1)) + (size_t)ny * k) + i])) * r2y;
+    if (!(f & 32)) gzp = (__ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k + 2) & (nz - 1))) + i]) - pc) * r2z;
+    if (!(f & 64)) gzm = (pc - __ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k - 2) & (nz - 1))) + i])) * r2z;
+    d[o] = dv + ((gxp - gxm) * r2x + (gyp - gym) * r2y + (gzp - gzm) * r2z);
 }
 
 // a6: u_a = beta ? u*_a - delta_a p : +0.0, in place (eq. 8)

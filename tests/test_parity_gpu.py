@@ -138,6 +138,28 @@ def test_per_stage_projection_variant():
         compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"flags=2 step {cp}")
 
 
+def test_eq9_sparse_list_and_dense_prologue_agree():
+    """eq. 9's right-hand side at the listed near-solid cells (default) and densely inside the forward x pass
+    (flags bit 2) are the same arithmetic: both match the oracle, and each other to rounding."""
+    case = cases.duct_room(64, 32, 32)
+    res = {}
+    for flags in (0, 4):
+        s = binding.solver_for_case(case, flags=flags)
+        n0 = s.launch_count()
+        s.step(3)
+        per_step = (s.launch_count() - n0) // 3
+        assert per_step == (4 + 1 + 4 * 6 + 1 if flags == 0 else 4 + 1 + 4 * 5 + 1)   # sparse: +1 launch per iteration
+        res[flags] = s.fields_numpy()
+        s.close()
+    o = oracle_for(case)
+    o.step(3)
+    ref = o.fields()
+    for flags in (0, 4):
+        compare(res[flags], ref, TOL1, mask=case["mask"], what=f"eq9 flags={flags}")
+    for k in "uvwcp":
+        assert relerr(res[0][k], res[4][k]) <= 1e-13
+
+
 def test_smooth_tanh_sources_and_body_force_unequal_spacing():
     case = cases.duct_room(32, 16, 16)
     case["d"] = (0.05, 0.07, 0.06)
