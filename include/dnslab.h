@@ -58,7 +58,9 @@ typedef struct {
     uint32_t flags;        /* bit0 reserved (eq. 6 filter, not built); bit1: project every RK stage;
                               bit2: evaluate eq. 9's right-hand side densely inside the forward x pass
                               instead of at the listed near-solid cells (same result; the library does
-                              this by itself when more than half of the cells are near-solid)         */
+                              this by itself when more than half of the cells are near-solid);
+                              bit3: two RK stages per launch (k_rk_pair: the intermediate stage field
+                              stays in shared memory; same result up to rounding; experimental)       */
 } dnslab_params_t;
 
 /* One inflow/outflow forcing region S(x,y,z) of eqs. 2-3. */

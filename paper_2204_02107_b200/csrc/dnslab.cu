@@ -28,7 +28,7 @@ bool valid_params(const dnslab_params_t *P)
     if (P->nx < 8 || P->nx > 2048 || P->ny < 8 || P->ny > 1024 || P->nz < 8 || P->nz > 1024) return false;
     if (!(P->dx > 0) || !(P->dy > 0) || !(P->dz > 0) || !(P->dt > 0)) return false;
     if (!(P->nu >= 0) || !(P->alpha_c >= 0) || P->n_piter < 1) return false;
-    if (P->flags & ~6u) return false;
+    if (P->flags & ~14u) return false;
     return true;
 }
 
@@ -110,6 +110,7 @@ struct dnslab {
     int64_t launches;
     dim3 rk_block;
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
+    int pair_kc; // > 0: two-stage kernel (k_rk_pair) with this many planes per block; 0: one launch per stage
     // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
     bool prof_on;
     std::vector<ProfRec> *prof;
@@ -200,6 +201,11 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
     a.rxx = 1.0 / (h->P.dx * h->P.dx); a.ryy = 1.0 / (h->P.dy * h->P.dy); a.rzz = 1.0 / (h->P.dz * h->P.dz);
     a.nu = h->P.nu; a.ac = h->P.alpha_c;
     for (int m = 0; m < 3; ++m) a.body[m] = h->P.body[m];
+    a.kf.hx = -0.5 * a.r2x; a.kf.hy = -0.5 * a.r2y; a.kf.hz = -0.5 * a.r2z;
+    a.kf.dvx = a.nu * a.rxx; a.kf.dvy = a.nu * a.ryy; a.kf.dvz = a.nu * a.rzz;
+    a.kf.dcx = a.ac * a.rxx; a.kf.dcy = a.ac * a.ryy; a.kf.dcz = a.ac * a.rzz;
+    a.kf.dv0 = -2.0 * (a.kf.dvx + a.kf.dvy + a.kf.dvz);
+    a.kf.dc0 = -2.0 * (a.kf.dcx + a.kf.dcy + a.kf.dcz);
     a.ca = ca[STAGE - 1] * h->P.dt;
     a.cb = cb[STAGE - 1] * h->P.dt;
     a.nsrc = h->nsrc;
@@ -233,6 +239,54 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
     else if (masked) dnsst::k_rk<STAGE, ELIM, true, false><<<grd, blk, 0, h->stream>>>(a);
     else if (sources) dnsst::k_rk<STAGE, ELIM, false, true><<<grd, blk, 0, h->stream>>>(a);
     else dnsst::k_rk<STAGE, ELIM, false, false><<<grd, blk, 0, h->stream>>>(a);
+    return check_launch(h);
+}
+
+// Two stages per launch (k_rk_pair): PAIR 0 = stages 1+2 (Qn -> Q2, Q3), PAIR 1 = stages 3+4 (Q3, Qn, Q2 -> Q* in place of Q2)
+template <int PAIR> int launch_rk_pair(dnslab *h, double *const *qs, double *const *q2, double *const *q3)
+{
+    dnsst::RKArgs a;
+    std::memset(&a, 0, sizeof(a));
+    for (int m = 0; m < 4; ++m) {
+        a.qs[m] = qs[m];
+        a.qn[m] = h->Q[m];
+        a.qc[m] = q2[m];
+        a.qo[m] = q2[m];
+        a.qco[m] = PAIR == 0 ? q3[m] : q2[m];
+    }
+    a.face = h->face;
+    a.nx = h->P.nx; a.ny = h->P.ny; a.nz = h->P.nz;
+    a.r2x = 1.0 / (2.0 * h->P.dx); a.r2y = 1.0 / (2.0 * h->P.dy); a.r2z = 1.0 / (2.0 * h->P.dz);
+    a.rxx = 1.0 / (h->P.dx * h->P.dx); a.ryy = 1.0 / (h->P.dy * h->P.dy); a.rzz = 1.0 / (h->P.dz * h->P.dz);
+    a.nu = h->P.nu; a.ac = h->P.alpha_c;
+    for (int m = 0; m < 3; ++m) a.body[m] = h->P.body[m];
+    a.kf.hx = -0.5 * a.r2x; a.kf.hy = -0.5 * a.r2y; a.kf.hz = -0.5 * a.r2z;
+    a.kf.dvx = a.nu * a.rxx; a.kf.dvy = a.nu * a.ryy; a.kf.dvz = a.nu * a.rzz;
+    a.kf.dcx = a.ac * a.rxx; a.kf.dcy = a.ac * a.ryy; a.kf.dcz = a.ac * a.rzz;
+    a.kf.dv0 = -2.0 * (a.kf.dvx + a.kf.dvy + a.kf.dvz);
+    a.kf.dc0 = -2.0 * (a.kf.dcx + a.kf.dcy + a.kf.dcz);
+    a.ca = (PAIR == 0 ? 0.5 : 1.0) * h->P.dt;
+    a.cb = (PAIR == 0 ? 0.5 : 1.0 / 6.0) * h->P.dt;
+    a.nsrc = h->nsrc;
+    a.stab = h->stab;
+    for (int s = 0; s < h->nsrc; ++s) a.src[s] = h->src[s];
+    a.kc = h->pair_kc;
+    const bool masked = h->face != nullptr, sources = h->nsrc > 0;
+    const dim3 grd(h->P.nx / dnsst::P2_TX, h->P.ny / dnsst::P2_TY, h->P.nz / h->pair_kc);
+    const size_t smem = PAIR == 0 ? dnsst::P2_SMEM0 : dnsst::P2_SMEM1;
+    ProfScope ps(h, DNSLAB_K_RK);
+#define DNS_LAUNCH_PAIR(M, S)                                                                                    \
+    do {                                                                                                         \
+        auto kern = dnsst::k_rk_pair<PAIR, M, S>;                                                                \
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)   \
+            return DNSLAB_ECUDA;                                                                                 \
+        kern<<<grd, dnsst::P2_NT, smem, h->stream>>>(a);                                                         \
+    } while (0)
+    if (masked && sources) DNS_LAUNCH_PAIR(true, true);
+    else if (masked) DNS_LAUNCH_PAIR(true, false);
+    else if (sources) DNS_LAUNCH_PAIR(false, true);
+    else DNS_LAUNCH_PAIR(false, false);
+#undef DNS_LAUNCH_PAIR
     return check_launch(h);
 }
 
@@ -485,6 +539,18 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
             }
             h->rk_kc = kc;
         }
+        // two stages per launch (flags bit 3) for nx >= 32, ny >= 16: one block per SM, >= 6 waves, at least 8 planes each
+        h->pair_kc = 0;
+        if (params->nx >= dnsst::P2_TX && params->ny >= dnsst::P2_TY && ((params->flags & 8u) || getenv("DNSLAB_RK_PAIR"))) {
+            const long tiles = (long)(params->nx / dnsst::P2_TX) * (params->ny / dnsst::P2_TY);
+            int kc = params->nz;
+            while (kc > 8 && tiles * (params->nz / kc) < 6L * prop.multiProcessorCount) kc /= 2;
+            if (const char *v = getenv("DNSLAB_PAIR_KC")) {
+                const int e = atoi(v);
+                if (e >= 1 && e <= params->nz && params->nz % e == 0) kc = e;
+            }
+            h->pair_kc = kc;
+        }
     }
 
     auto fail = [&](int rc) { delete h; return rc; };
@@ -616,12 +682,18 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
     const size_t bytes = h->n * sizeof(double);
     int rc;
     for (int it = 0; it < nsteps; ++it) {
-        if (!stage_proj) {
+        if (!stage_proj && h->pair_kc > 0) {
+            // two launches: stages 1+2 (A = Q2, Bf = Q3), stages 3+4 (Q4 stays on chip, Q* overwrites A)
+            if ((rc = launch_rk_pair<0>(h, h->Q, h->A, h->Bf))) return rc;
+            if ((rc = launch_rk_pair<1>(h, h->Bf, h->A, h->Bf))) return rc;
+        } else if (!stage_proj) {
             // Qc eliminated: A = Q2 (then Q*), Bf = Q3, Qc = Q4
             if ((rc = launch_rk<1, true>(h, h->Q, h->A, nullptr, nullptr))) return rc;
             if ((rc = launch_rk<2, true>(h, h->A, h->Bf, nullptr, nullptr))) return rc;
             if ((rc = launch_rk<3, true>(h, h->Bf, h->Qc, nullptr, nullptr))) return rc;
             if ((rc = launch_rk<4, true>(h, h->Qc, nullptr, h->A, h->Bf))) return rc;
+        }
+        if (!stage_proj) {
             if ((rc = pressure_stage(h, h->A, h->p))) return rc;
             for (int m = 0; m < 4; ++m) {
                 double *t = h->Q[m];

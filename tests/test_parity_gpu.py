@@ -32,7 +32,7 @@ def compare(got, ref, tol, mask=None, what=""):
 
 def run_both(case, checkpoints, n_piter=None, flags=0):
     s = binding.solver_for_case(case, n_piter=n_piter, flags=flags)
-    o = oracle_for(case, n_piter=n_piter, flags=flags)
+    o = oracle_for(case, n_piter=n_piter, flags=flags & 2)   # only bit 1 changes the method; the rest pick kernels
     done = 0
     for cp in checkpoints:
         s.step(cp - done)
@@ -136,6 +136,20 @@ def test_per_stage_projection_variant():
     case = cases.duct_room(32, 16, 16)
     for cp, got, ref in run_both(case, [1, 5], flags=2):
         compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"flags=2 step {cp}")
+
+
+def test_two_stage_rk_kernel_variant():
+    """flags bit 3: stages 1+2 and 3+4 fused (k_rk_pair, intermediate stage field in shared memory) -- same method,
+    same tolerances; masked with sources, unmasked, a grid of one tile in x, and a z extent of one chunk."""
+    for case, cps in [(cases.duct_room(64, 32, 32), [1, 20]), (cases.config(1), [1, 10]), (cases.duct_room(32, 16, 8), [1, 3])]:
+        for cp, got, ref in run_both(case, cps, flags=8):
+            compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"flags=8 {case['name']} step {cp}")
+    case = cases.duct_room(64, 32, 32)
+    s = binding.solver_for_case(case, flags=8)
+    n0 = s.launch_count()
+    s.step(1)
+    assert s.launch_count() - n0 == 2 + 1 + 4 * 6 + 1
+    s.close()
 
 
 def test_eq9_sparse_list_and_dense_prologue_agree():
