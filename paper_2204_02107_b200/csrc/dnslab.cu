@@ -109,6 +109,7 @@ struct dnslab {
     dnsst::SourceDev src[DNSLAB_MAX_SOURCES];
     int64_t launches;
     dim3 rk_block;
+    int nsm;   // SM count of the device
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
     int pair_kc; // > 0: two-stage kernel (k_rk_pair) with this many planes per block; 0: one launch per stage
     // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
@@ -293,6 +294,22 @@ template <int PAIR> int launch_rk_pair(dnslab *h, double *const *qs, double *con
 // ---- FFT passes -------------------------------------------------------------------------
 template <int L> constexpr int col_xt() { return L >= 1024 ? 4 : (L >= 256 ? 8 : 16); }
 
+// grid of a persistent pass: every SM filled with as many blocks as fit, never more blocks than tiles
+template <typename K> int persistent_grid(dnslab *h, K kernel, int threads, size_t smem, size_t ntiles, unsigned *grid)
+{
+    if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem));
+    if (per_sm < 1) return DNSLAB_ECUDA;
+    size_t g = (size_t)per_sm * h->nsm;
+    if (g > ntiles) g = ntiles;
+    // equal shares: the smallest grid that still needs the same number of tiles per block
+    const size_t per_block = (ntiles + g - 1) / g;
+    g = (ntiles + per_block - 1) / per_block;
+    *grid = (unsigned)g;
+    return DNSLAB_OK;
+}
+
 template <int L, int DIR, bool PRO> int launch_fft_x_L(dnslab *h, const c2 *in, c2 *out, const dnsfft::PoissonRhsArgs &ra)
 {
     constexpr int E = dnsfft::ElemsPerThread<L>::value;
@@ -322,12 +339,6 @@ template <int DIR, bool PRO> int launch_fft_x(dnslab *h, const c2 *in, c2 *out, 
     return DNSLAB_EINVAL;
 }
 
-template <typename K> int set_smem(K kernel, size_t smem)
-{
-    if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    return DNSLAB_OK;
-}
-
 // y pass: axis 1; z pass (unfused, used only by tests of the transform itself): axis 2
 template <int L, int XT, int DIR> int launch_fft_col_LX(dnslab *h, c2 *data, int axis)
 {
@@ -338,7 +349,7 @@ template <int L, int XT, int DIR> int launch_fft_col_LX(dnslab *h, c2 *data, int
     const int nother = axis == 1 ? h->P.nz : h->P.ny;
     const size_t smem = (size_t)XT * L * sizeof(c2);
     auto kern = dnsfft::k_fft_col<L, XT, DIR>;
-    if (int rc = set_smem(kern, smem)) return rc;
+    if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ProfScope ps(h, DNSLAB_K_FFT_Y);
     kern<<<(unsigned)((mx / XT) * nother), XT * T, smem, h->stream>>>(data, h->tw[axis], mx, stride, other_stride);
     return check_launch(h);
@@ -369,13 +380,16 @@ template <int DIR> int launch_fft_col(dnslab *h, c2 *data, int axis)
 template <int L, int XT> int launch_fft_z_solve_LX(dnslab *h, c2 *data)
 {
     constexpr int T = L / dnsfft::ElemsPerThread<L>::value;
+    constexpr int NT = XT * T < 32 ? 32 : XT * T;
     const int mx = h->P.nx / 2;
-    const size_t smem = (size_t)XT * L * sizeof(c2);
+    const size_t smem = 2 * (size_t)XT * L * sizeof(c2);
+    const size_t ntiles = (size_t)(mx / XT) * h->P.ny;
     auto kern = dnsfft::k_fft_z_solve<L, XT>;
-    if (int rc = set_smem(kern, smem)) return rc;
+    unsigned grid = 0;
+    if (int rc = persistent_grid(h, kern, NT, smem, ntiles, &grid)) return rc;
     ProfScope ps(h, DNSLAB_K_FFT_Z);
     const double inv_n = 2.0 / (double)h->n; // the packed transform has n/2 complex points
-    kern<<<(unsigned)((mx / XT) * h->P.ny), XT * T, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], inv_n);
+    kern<<<grid, XT * T, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], inv_n, (int)ntiles);
     return check_launch(h);
 }
 
@@ -506,6 +520,7 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
     h->P = *params;
     h->n = (size_t)params->nx * params->ny * params->nz;
     h->stream = (cudaStream_t)cuda_stream;
+    h->nsm = prop.multiProcessorCount;
     h->ws = (char *)workspace;
     h->L = make_layout(params);
     const Layout &L = h->L;

@@ -109,7 +109,7 @@ template <int L, int E, int NS> struct NextRadix {
 
 // Full transform of one line held as x[e] <-> element tid + e*T, exchanging through `sm`
 // (SM::at(n) gives a reference to the shared slot of logical element n of this thread's line).
-// All threads of the block must call this together (it contains __syncthreads()).
+// All threads that share the view must call this together (sm.sync() is a barrier among them).
 template <int L, int E, int DIR, int NS, class SM> __device__ __forceinline__ void fft_line(c2 (&x)[E], int tid, const c2 *__restrict__ tw, SM &sm)
 {
     constexpr int T = L / E;
@@ -125,24 +125,33 @@ template <int L, int E, int DIR, int NS, class SM> __device__ __forceinline__ vo
 #pragma unroll
             for (int r = 0; r < R; ++r) sm.at(j0 + r * NS) = x[q + r * Q];
         }
-        __syncthreads();
+        sm.sync();
 #pragma unroll
         for (int e = 0; e < E; ++e) x[e] = sm.at(tid + e * T);
-        __syncthreads();
+        sm.sync();
         fft_line<L, E, DIR, NS * R, SM>(x, tid, tw, sm);
     }
 }
 
 // shared-memory views -------------------------------------------------------------------
 // contiguous line with one pad element per 8 (x pass: threads of a warp walk along the line)
-struct SmLine {
+// The T threads of a line are T consecutive threads: inside one warp for T <= 32 (__syncwarp), else a
+// named barrier per line (id 1 + line-in-block, at most 15 lines per block then).
+template <int T> struct SmLine {
     c2 *base;
+    int bar;
     __device__ __forceinline__ c2 &at(int n) { return base[n + (n >> 3)]; }
+    __device__ __forceinline__ void sync()
+    {
+        if constexpr (T <= 32) __syncwarp();
+        else asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(T) : "memory");
+    }
 };
 // column of a tile whose fastest index is the XT-wide x offset (y and z passes)
 template <int XT> struct SmCol {
     c2 *base; // already offset by tx
     __device__ __forceinline__ c2 &at(int n) { return base[n * XT]; }
+    __device__ __forceinline__ void sync() { __syncthreads(); }
 };
 
 template <int L> struct ElemsPerThread { static constexpr int value = L >= 8 ? 8 : L; };
@@ -177,9 +186,22 @@ __device__ __forceinline__ double eq9_rhs(const PoissonRhsArgs &a, double dv, in
 }
 
 // ---------------------------------------------------------------------------------------
-// x pass: lines of L = nx/2 complex numbers, contiguous.  NL lines per block.
+// The fused z pass is persistent: a block walks tiles blockIdx.x, blockIdx.x + gridDim.x, ... and keeps the
+// NEXT tile in flight (cp.async, 16 bytes per complex element, into the other of two shared-memory
+// buffers) while it transforms the current one.  Every thread copies exactly the elements it will hold
+// in registers, so reading them back needs only cp.async.wait_group; the buffer then serves as the
+// exchange area of the radix stages (one __syncthreads first: other threads' slots are overwritten).
+__device__ __forceinline__ void cp_async_c2(c2 *dst_smem, const c2 *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
+
+// x pass: lines of L = nx/2 complex numbers, contiguous.  NL lines per block, one line per T consecutive
+// threads, so the exchanges of a line never leave its warp (or its named barrier).
 //   FWD with PROLOGUE: in = d (real array viewed as complex), r = eq9_rhs(...) computed on load.
-//   out-of-place or in-place (a block reads its lines completely before it writes them).
+//   out-of-place or in-place (a line is read completely before it is written).
 template <int L, int DIR, bool PROLOGUE>
 __global__ void __launch_bounds__(256) k_fft_x(const c2 *__restrict__ in, c2 *__restrict__ out, const c2 *__restrict__ tw, int nlines_per_block,
                                                PoissonRhsArgs ra)
@@ -207,8 +229,8 @@ __global__ void __launch_bounds__(256) k_fft_x(const c2 *__restrict__ in, c2 *__
             }
         }
     }
-    SmLine sm{smem + lt * (L + L / 8)};
-    fft_line<L, E, DIR, 1, SmLine>(x, tid, tw, sm);
+    SmLine<T> sm{smem + lt * (L + L / 8), 1 + lt};
+    fft_line<L, E, DIR, 1, SmLine<T>>(x, tid, tw, sm);
     c2 *dst = out + line * L;
 #pragma unroll
     for (int e = 0; e < E; ++e) dst[tid + e * T] = x[e];
@@ -241,11 +263,11 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThread<L>::value) < 32 ? 32 :
 // Fused middle pass along z: forward transform, division by the modified-wavenumber eigenvalue
 //   lambda(m,ky,kz) = -(ex[m] + ey[ky] + ez[kz]),  e_a[k] = (sin(2 pi k/N_a)/D_a)^2,
 // null modes (m = 0, 2ky = 0 mod ny, 2kz = 0 mod nz) set to 0, scaling by 1/N, inverse transform.
-// blockIdx.x enumerates (x tile, ky).
+// The tile index enumerates (x tile, ky).
 template <int L, int XT>
 __global__ void __launch_bounds__(XT *(L / ElemsPerThread<L>::value) < 32 ? 32 : XT *(L / ElemsPerThread<L>::value))
     k_fft_z_solve(c2 *__restrict__ data, const c2 *__restrict__ tw, int mx, int ny, const double *__restrict__ ex,
-                  const double *__restrict__ ey, const double *__restrict__ ez, double inv_n)
+                  const double *__restrict__ ey, const double *__restrict__ ez, double inv_n, int ntiles)
 {
     constexpr int E = ElemsPerThread<L>::value;
     constexpr int T = L / E;
@@ -253,31 +275,47 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThread<L>::value) < 32 ? 32 :
     const int tx = threadIdx.x % XT;
     const int tid = threadIdx.x / XT;
     const int xtiles = mx / XT;
-    const int xt = blockIdx.x % xtiles;
-    const int ky = blockIdx.x / xtiles;
-    const int m = xt * XT + tx;
     const size_t stride = (size_t)mx * ny;
-    c2 *base = data + (size_t)ky * mx + m;
-    c2 x[E];
+    auto issue = [&](int tile, int b) {
+        const c2 *src = data + (size_t)(tile / xtiles) * mx + (tile % xtiles) * XT + tx;
+        c2 *dst = smem + b * (XT * L) + tx;
 #pragma unroll
-    for (int e = 0; e < E; ++e) x[e] = base[(size_t)(tid + e * T) * stride];
-    SmCol<XT> sm{smem + tx};
-    fft_line<L, E, -1, 1, SmCol<XT>>(x, tid, tw, sm);
-    const double exy = __ldg(&ex[m]) + __ldg(&ey[ky]);
-    const bool null_xy = (m == 0) && (((2 * ky) & (ny - 1)) == 0);
+        for (int e = 0; e < E; ++e) cp_async_c2(&dst[(tid + e * T) * XT], &src[(size_t)(tid + e * T) * stride]);
+    };
+    double ezr[E]; // 1/N scaling folded in later; ez depends only on this thread's kz
 #pragma unroll
-    for (int e = 0; e < E; ++e) {
-        const int kz = tid + e * T;
-        const double lam = -(exy + __ldg(&ez[kz]));
-        const bool null = null_xy && (((2 * kz) & (L - 1)) == 0);
-        const double s = null ? 0.0 : inv_n / lam;
-        x[e].x = null ? 0.0 : x[e].x * s;
-        x[e].y = null ? 0.0 : x[e].y * s;
+    for (int e = 0; e < E; ++e) ezr[e] = __ldg(&ez[tid + e * T]);
+    int tile = blockIdx.x, b = 0;
+    if (tile < ntiles) issue(tile, 0);
+    cp_async_commit();
+    for (; tile < ntiles; tile += gridDim.x, b ^= 1) {
+        if (tile + (int)gridDim.x < ntiles) issue(tile + gridDim.x, b ^ 1);
+        cp_async_commit();
+        cp_async_wait_1();
+        const int ky = tile / xtiles, m = (tile % xtiles) * XT + tx;
+        SmCol<XT> sm{smem + b * (XT * L) + tx};
+        c2 x[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = sm.at(tid + e * T);
+        __syncthreads();
+        fft_line<L, E, -1, 1, SmCol<XT>>(x, tid, tw, sm);
+        const double exy = __ldg(&ex[m]) + __ldg(&ey[ky]);
+        const bool null_xy = (m == 0) && (((2 * ky) & (ny - 1)) == 0);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int kz = tid + e * T;
+            const double lam = -(exy + ezr[e]);
+            const bool null = null_xy && (((2 * kz) & (L - 1)) == 0);
+            const double s = null ? 0.0 : inv_n / lam;
+            x[e].x = null ? 0.0 : x[e].x * s;
+            x[e].y = null ? 0.0 : x[e].y * s;
+        }
+        __syncthreads();
+        fft_line<L, E, +1, 1, SmCol<XT>>(x, tid, tw, sm);
+        c2 *base = data + (size_t)ky * mx + m;
+#pragma unroll
+        for (int e = 0; e < E; ++e) base[(size_t)(tid + e * T) * stride] = x[e];
     }
-    __syncthreads();
-    fft_line<L, E, +1, 1, SmCol<XT>>(x, tid, tw, sm);
-#pragma unroll
-    for (int e = 0; e < E; ++e) base[(size_t)(tid + e * T) * stride] = x[e];
 }
 
 } // namespace dnsfft
