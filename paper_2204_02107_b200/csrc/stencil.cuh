@@ -178,15 +178,15 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
 // k_rk_march: the same stage (a1-a3) for grids with nx >= 64, marching along z.
 //
 // A block owns a 64 x 8 (x by y) column of cells and walks kc planes of it.  Each thread owns two
-// x-adjacent cells (one double2 per field).  The stage field's plane k+2 is in flight (cp.async,
-// LDGSTS) into one of three shared-memory plane tiles (4 fields x 10 rows x 64+2 cells, halo included,
+// x-adjacent cells (one double2 per field).  The stage field's planes k+2 and k+3 are in flight (cp.async,
+// LDGSTS) into two of four shared-memory plane tiles (4 fields x 10 rows x 64+2 cells, halo included,
 // periodic wrap applied to the source address) while plane k is being computed: x/y neighbours come
 // from the tile of plane k, the z+1 neighbour from the tile of plane k+1, the z-1 neighbour and the
 // centre are carried in registers.  So every stage-field value is fetched from L2/HBM once per block
 // (plus the one-cell halo), the bytes in flight live in shared memory rather than in registers, and
 // the other operands (Qn, Q2, Q3) and the result are streamed as 16-byte accesses.
 // One __syncthreads per plane.  Arithmetic and select semantics are those of k_rk above.
-constexpr int RKM_TX = 64, RKM_TY = 8, RKM_SW = 68, RKM_ROWS = RKM_TY + 2, RKM_NBUF = 3;
+constexpr int RKM_TX = 64, RKM_TY = 8, RKM_SW = 68, RKM_ROWS = RKM_TY + 2, RKM_NBUF = 4;
 constexpr int RKM_SMEM = RKM_NBUF * 4 * RKM_ROWS * RKM_SW * (int)sizeof(double);
 
 __device__ __forceinline__ void cp_async16(void *dst_smem, const void *src)
@@ -199,6 +199,7 @@ __device__ __forceinline__ void cp_async8(void *dst_smem, const void *src)
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_one() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
 
 // RHS of one cell for field m given its seven-point neighbourhood and the advecting velocities.
 template <bool MASKED_C>
@@ -261,6 +262,7 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
 
     issue_plane(k0, 0);
     issue_plane(k0 + 1, 1);
+    issue_plane(k0 + 2, 2);
     double2 zm[4], cur[4];
     {
         const size_t pkm = plane * (size_t)((k0 - 1) & (nz - 1));
@@ -289,9 +291,10 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
                 q3[m] = __ldg(reinterpret_cast<const double2 *>(a.q3[m] + o));
             }
         }
-        cp_async_wait_all();
+        cp_async_wait_one();
         __syncthreads(); // plane k+1 visible to all; every thread is done with the tile of plane k-1
-        if (t + 2 <= kc) issue_plane(k + 2, (t + 2) % RKM_NBUF);
+        if (t + 3 <= kc) issue_plane(k + 3, (t + 3) % RKM_NBUF);
+        else cp_async_commit();
         const double *sC = sm + (t % RKM_NBUF) * PLANE, *sN = sm + ((t + 1) % RKM_NBUF) * PLANE;
         if (t == 0) {
 #pragma unroll
@@ -554,7 +557,6 @@ __device__ __forceinline__ void pair_rhs(const RKArgs &a, const PairCoef &k, con
     }
 #pragma unroll
     for (int m = 0; m < 3; ++m) {
-        asm volatile("" ::: "memory");
         double xp[2], xm[2], yp[2], ym[2];
         pair_nb(tile + m * FS, offL, offR, split, q0[m], xp, xm, yp, ym);
 #pragma unroll
@@ -639,7 +641,7 @@ template <int PAIR, bool MASKED, bool SOURCES> __global__ void __launch_bounds__
         colR = P2_W - 2;
     }
     const int gj = (y0 - 1 + ar) & (ny - 1), giL = (x0 - 2 + colL) & (nx - 1), giR = (x0 - 2 + colR) & (nx - 1);
-    const size_t ocL = (size_t)nx * gj + giL, ocR = (size_t)nx * gj + giR; // offsets of the two columns inside a plane
+    const unsigned ocL = (unsigned)nx * gj + giL, ocR = (unsigned)nx * gj + giR; // offsets of the two columns inside a plane
     const int qL = (ar + 1) * P2_W + colL, qR = (ar + 1) * P2_W + colR;    // inside a field of a stage-A input tile
     const int aL = ar * P2_W + colL, aR = ar * P2_W + colR;                // inside a field of an A' (or Qn) tile
 
@@ -648,8 +650,8 @@ template <int PAIR, bool MASKED, bool SOURCES> __global__ void __launch_bounds__
     const int t1 = t + P2_NT, lr1 = t1 / (P2_W / 2), lc1 = t1 - lr1 * (P2_W / 2);
     const bool hasL1 = t1 < P2_CHUNKS, hasN0 = t < P2_ACHUNKS, hasN1 = t1 < P2_ACHUNKS;
     const int lx0 = (x0 - 2 + 2 * lc0) & (nx - 1), lx1 = (x0 - 2 + 2 * lc1) & (nx - 1);
-    const size_t ls0 = (size_t)nx * ((y0 - 2 + lr0) & (ny - 1)) + lx0, ls1 = (size_t)nx * ((y0 - 2 + lr1) & (ny - 1)) + lx1;
-    const size_t ns0 = (size_t)nx * ((y0 - 1 + lr0) & (ny - 1)) + lx0, ns1 = (size_t)nx * ((y0 - 1 + lr1) & (ny - 1)) + lx1;
+    const unsigned ls0 = (unsigned)nx * ((y0 - 2 + lr0) & (ny - 1)) + lx0, ls1 = (unsigned)nx * ((y0 - 2 + lr1) & (ny - 1)) + lx1;
+    const unsigned ns0 = (unsigned)nx * ((y0 - 1 + lr0) & (ny - 1)) + lx0, ns1 = (unsigned)nx * ((y0 - 1 + lr1) & (ny - 1)) + lx1;
     const int ld0 = lr0 * P2_W + 2 * lc0, ld1 = lr1 * P2_W + 2 * lc1;
     // stage-A input plane k0-2+n into tile n % 4; PAIR 1: Qn at plane k0-1+sn (stage-A plane of iteration sn) into tile phn
     auto issue_planes = [&](int n, bool doq, int sn, int phn, bool don) {
@@ -688,20 +690,19 @@ template <int PAIR, bool MASKED, bool SOURCES> __global__ void __launch_bounds__
     issue_planes(2, true, 1, 1, true);
     issue_planes(3, true, 0, 0, false);
 
-    auto ld_face = [&](size_t pk, unsigned (&f)[2]) {
+    // face bytes of the two cells, fetched one iteration ahead and left packed until they are used
+    auto ld_face = [&](size_t pk, unsigned (&raw)[2]) {
         if (!split) {
-            const uchar2 v = *reinterpret_cast<const uchar2 *>(a.face + pk + ocL);
-            f[0] = v.x;
-            f[1] = v.y;
+            raw[0] = *reinterpret_cast<const unsigned short *>(a.face + pk + ocL);
         } else {
-            f[0] = a.face[pk + ocL];
-            f[1] = a.face[pk + ocR];
+            raw[0] = a.face[pk + ocL];
+            raw[1] = a.face[pk + ocR];
         }
     };
 
     // z-carried registers: three rotating sets for the stage-A input column
     pair4 R0, R1, R2;
-    unsigned fA[2] = {0x7f, 0x7f}, fB[2] = {0x7f, 0x7f}, fN[2] = {0x7f, 0x7f};
+    unsigned fA[2] = {0x7f, 0x7f}, fB[2] = {0x7f, 0x7f}, fN[2] = {0x7f7f, 0x7f};
 #pragma unroll
     for (int m = 0; m < 4; ++m)
 #pragma unroll
@@ -726,7 +727,8 @@ template <int PAIR, bool MASKED, bool SOURCES> __global__ void __launch_bounds__
     auto body = [&](const int s, const int ph, pair4 &Azm, pair4 &Ac, pair4 &Azp) {
         const int ka = (k0 - 1 + s) & (nz - 1), kb = (ka - 1) & (nz - 1);
         fB[0] = fA[0]; fB[1] = fA[1];
-        fA[0] = fN[0]; fA[1] = fN[1];
+        fA[0] = split ? fN[0] : (fN[0] & 0xffu);
+        fA[1] = split ? fN[1] : (fN[0] >> 8);
         if (MASKED && hasA && s <= kc) ld_face(plane * (size_t)((ka + 1) & (nz - 1)), fN);
         double2 rb[4]; // PAIR 1: R at the stage-B plane, consumed at the very end of the iteration
         if (PAIR == 1 && interior && s >= 2) {
