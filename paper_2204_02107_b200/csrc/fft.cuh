@@ -75,7 +75,7 @@ template <int DIR> __device__ __forceinline__ void dft8(c2 (&v)[8])
 // One Stockham stage of radix R on the E register elements of thread `tid` (element e <-> index
 // tid + e*T).  Ns = product of the radices of the earlier stages.  On exit slot q + r*(E/R) holds
 // output r of butterfly jj = tid + q*T, whose natural position is oidx = expand(jj) + r*Ns.
-template <int L, int E, int R, int NS, int DIR> __device__ __forceinline__ void stage(c2 (&x)[E], int tid, const c2 *__restrict__ tw)
+template <int L, int E, int R, int NS, int DIR, bool TWPOW> __device__ __forceinline__ void stage(c2 (&x)[E], int tid, const c2 *__restrict__ tw)
 {
     constexpr int T = L / E;
     constexpr int Q = E / R;
@@ -87,8 +87,25 @@ template <int L, int E, int R, int NS, int DIR> __device__ __forceinline__ void 
         if constexpr (NS > 1) {
             const int jm = (tid + q * T) & (NS - 1);
             const int kb = jm * (L / (NS * R));
+            if constexpr (TWPOW && R > 2) {
+                // one table look-up per butterfly, the other twiddles as its powers (product depth <= 3):
+                // lanes of a warp hold different jm in the x pass, so each look-up is a gather
+                c2 w[R];
+                w[1] = __ldg(&tw[kb]);
+                w[2] = cmul(w[1], w[1]);
+                w[3] = cmul(w[2], w[1]);
+                if constexpr (R == 8) {
+                    w[4] = cmul(w[2], w[2]);
+                    w[5] = cmul(w[4], w[1]);
+                    w[6] = cmul(w[4], w[2]);
+                    w[7] = cmul(w[4], w[3]);
+                }
 #pragma unroll
-            for (int r = 1; r < R; ++r) v[r] = twmul<DIR>(v[r], __ldg(&tw[kb * r]));
+                for (int r = 1; r < R; ++r) v[r] = twmul<DIR>(v[r], w[r]);
+            } else {
+#pragma unroll
+                for (int r = 1; r < R; ++r) v[r] = twmul<DIR>(v[r], __ldg(&tw[kb * r]));
+            }
         }
         if constexpr (R == 8) {
             dft8<DIR>(v);
@@ -115,7 +132,7 @@ template <int L, int E, int DIR, int NS, class SM> __device__ __forceinline__ vo
     constexpr int T = L / E;
     constexpr int R = NextRadix<L, E, NS>::value;
     constexpr int Q = E / R;
-    stage<L, E, R, NS, DIR>(x, tid, tw);
+    stage<L, E, R, NS, DIR, SM::TWPOW>(x, tid, tw);
     if constexpr (NS * R < L) {
 #pragma unroll
         for (int q = 0; q < Q; ++q) {
@@ -138,6 +155,7 @@ template <int L, int E, int DIR, int NS, class SM> __device__ __forceinline__ vo
 // The T threads of a line are T consecutive threads: inside one warp for T <= 32 (__syncwarp), else a
 // named barrier per line (id 1 + line-in-block, at most 15 lines per block then).
 template <int T> struct SmLine {
+    static constexpr bool TWPOW = true;
     c2 *base;
     int bar;
     __device__ __forceinline__ c2 &at(int n) { return base[n + (n >> 3)]; }
@@ -149,6 +167,7 @@ template <int T> struct SmLine {
 };
 // column of a tile whose fastest index is the XT-wide x offset (y and z passes)
 template <int XT> struct SmCol {
+    static constexpr bool TWPOW = false; // lanes share the twiddle here: XT adjacent x per radix position
     c2 *base; // already offset by tx
     __device__ __forceinline__ c2 &at(int n) { return base[n * XT]; }
     __device__ __forceinline__ void sync() { __syncthreads(); }
