@@ -41,7 +41,7 @@ typedef struct {
     double nu, alpha_c, dt;
     double body[3];
     int32_t n_piter; /* eq. 9 iterations, PAPER.md:104 (paper: 4) */
-    uint32_t flags;  /* bit0: reserved (eq. 6 filter, not built); bit1: project every RK stage */
+    uint32_t flags;  /* bit0: eq. 6 filter at the end of each step (NEXT-1); bit1: project every RK stage */
 } dnsref_params_t;
 
 typedef struct {
@@ -73,6 +73,7 @@ int dnsref_num_threads(void)
 }
 
 static inline int wrap(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); }
+static inline int wrapm(int i, int n) { return ((i % n) + n) % n; } /* any offset, any n >= 1 */
 #define IDX(i, j, k) ((int64_t)(i) + (int64_t)nx * ((int64_t)(j) + (int64_t)ny * (int64_t)(k)))
 
 /* ------------------------------------------------------------------------
@@ -349,6 +350,41 @@ void dnsref_project(const dnsref_t *h, const double *us, const double *vs, const
             }
 }
 
+/* NEXT-1, eq. 6: explicit filter applied "at the end of each timestep" to u, v, w, c:
+ *     out = beta ? in + sum_a gamma_a d6_a(in) : +0.0,     gamma_a = Delta_a^6 / pi^6  (as printed),
+ * with d6_a the 2nd-order central 7-point stencil of the sixth derivative along axis a,
+ *     d6_a f = (f[-3] - 6 f[-2] + 15 f[-1] - 20 f[0] + 15 f[+1] - 6 f[+2] + f[+3]) / Delta_a^6,
+ * periodic (reading R23 in DESIGN.md: the paper does not say how the derivative is taken; "2nd order
+ * central" is its stated discretisation).  Delta_a^6 cancels: the weight of each stencil
+ * sum is 1/pi^6.  The stencil reads solid cells (which hold +0.0) like any other cell; the result is
+ * masked by the select of PAPER.md:58.  A Fourier mode with angles theta_a is multiplied by
+ *     G = 1 - (64/pi^6) sum_a sin^6(theta_a/2)                                      (pin P15).
+ * in and out must not alias. */
+void dnsref_filter(const dnsref_t *h, const double *in, double *out)
+{
+    const int nx = h->P.nx, ny = h->P.ny, nz = h->P.nz;
+    const double pi = 3.14159265358979323846;
+    const double g = 1.0 / (pi * pi * pi * pi * pi * pi);
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const int64_t o = IDX(i, j, k);
+                if (!h->beta[o]) { out[o] = 0.0; continue; }
+                const double f0 = in[o];
+                const double sx = in[IDX(wrapm(i - 3, nx), j, k)] - 6.0 * in[IDX(wrapm(i - 2, nx), j, k)] +
+                                  15.0 * in[IDX(wrapm(i - 1, nx), j, k)] - 20.0 * f0 + 15.0 * in[IDX(wrapm(i + 1, nx), j, k)] -
+                                  6.0 * in[IDX(wrapm(i + 2, nx), j, k)] + in[IDX(wrapm(i + 3, nx), j, k)];
+                const double sy = in[IDX(i, wrapm(j - 3, ny), k)] - 6.0 * in[IDX(i, wrapm(j - 2, ny), k)] +
+                                  15.0 * in[IDX(i, wrapm(j - 1, ny), k)] - 20.0 * f0 + 15.0 * in[IDX(i, wrapm(j + 1, ny), k)] -
+                                  6.0 * in[IDX(i, wrapm(j + 2, ny), k)] + in[IDX(i, wrapm(j + 3, ny), k)];
+                const double sz = in[IDX(i, j, wrapm(k - 3, nz))] - 6.0 * in[IDX(i, j, wrapm(k - 2, nz))] +
+                                  15.0 * in[IDX(i, j, wrapm(k - 1, nz))] - 20.0 * f0 + 15.0 * in[IDX(i, j, wrapm(k + 1, nz))] -
+                                  6.0 * in[IDX(i, j, wrapm(k + 2, nz))] + in[IDX(i, j, wrapm(k + 3, nz))];
+                out[o] = f0 + g * ((sx + sy) + sz);
+            }
+}
+
 /* The pressure stage: divergence, n_piter iterations of eq. 9 warm-started
  * from p, then the correction.  us.. and u.. may alias. */
 static void pressure_stage(dnsref_t *h, double *us, double *vs, double *ws, double *p)
@@ -368,6 +404,7 @@ static void pressure_stage(dnsref_t *h, double *us, double *vs, double *ws, doub
  *   d = div(Qc); p <- eq. 9 x n_piter; u = beta ? Qc.u - grad p : 0; c = Qc.c
  * Classical RK4: a = (1/2,1/2,1), b = (1/6,1/3,1/3,1/6) (reading R1).
  * flags bit1 (NEXT-2): each stage field Qs (s = 2..4) is projected too.
+ * flags bit0 (NEXT-1): u, v, w, c are filtered (eq. 6) after the projection.
  * ---------------------------------------------------------------------- */
 int dnsref_step(dnsref_t *h, int nsteps)
 {
@@ -399,7 +436,8 @@ int dnsref_step(dnsref_t *h, int nsteps)
         }
         pressure_stage(h, h->qc[0], h->qc[1], h->qc[2], h->p);
         for (int m = 0; m < 4; ++m) {
-            memcpy(h->q[m], h->qc[m], sizeof(double) * n);
+            if (h->P.flags & 1u) dnsref_filter(h, h->qc[m], h->q[m]); /* eq. 6, end of step (NEXT-1) */
+            else memcpy(h->q[m], h->qc[m], sizeof(double) * n);
         }
     }
     return DNSREF_OK;

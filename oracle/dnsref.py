@@ -57,6 +57,8 @@ def lib():
         L.dnsref_div.restype = None
         L.dnsref_poisson_rhs.argtypes = [C.c_void_p] + [C.c_void_p] * 3
         L.dnsref_poisson_rhs.restype = None
+        L.dnsref_filter.argtypes = [C.c_void_p] + [C.c_void_p] * 2
+        L.dnsref_filter.restype = None
         L.dnsref_project.argtypes = [C.c_void_p] + [C.c_void_p] * 7
         L.dnsref_project.restype = None
         L.dnsref_fft1d.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_int]
@@ -179,6 +181,13 @@ class Oracle:
         r = self._new()
         lib().dnsref_poisson_rhs(self._h, _ptr(d), _ptr(p), _ptr(r))
         return r
+
+    def filter(self, f):
+        """eq. 6 on one field (masked by the select)."""
+        f = _f64(f)
+        out = self._new()
+        lib().dnsref_filter(self._h, _ptr(f), _ptr(out))
+        return out
 
     def project(self, us, vs, ws, p):
         a = [_f64(x) for x in (us, vs, ws, p)]

@@ -464,3 +464,64 @@ def test_momentum_drift_bound_full_step():
     f = _run_case(case, 1)
     for k in "uvw":
         assert 0 < abs(f[k].mean() - case[k].mean()) < 1e-4      # 32^3, k0 = 4: ~2e-5 u' per step
+
+
+# ---------------------------------------------------------------- eq. 6 filter (P15, NEXT-1)
+def test_P15_filter_mode_amplification_closed_form():
+    """A Fourier mode is multiplied by G = 1 - (64/pi^6) sum_a sin^6(theta_a/2): the symbol of the central
+    7-point sixth-derivative stencil times gamma_a = Delta_a^6/pi^6 (eq. 6); Delta cancels, so
+    unequal spacings give the same factor.  Constant fields pass unchanged; a one-axis Nyquist mode is
+    damped by 1 - 64/pi^6 (not zeroed: reading R23)."""
+    shape = (16, 8, 32)
+    nz, ny, nx = shape
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    for d in [(0.1, 0.1, 0.1), (0.05, 0.2, 0.13)]:
+        o = mk(shape, d)
+        for (kx, ky, kz, ph) in [(0, 0, 0, 0.3), (1, 0, 0, 0.0), (3, 2, 5, 0.7), (nx // 2, 0, 0, 0.0), (nx // 2, ny // 2, nz // 2, 0.0),
+                                 (nx // 4, ny // 4, 1, 1.1)]:
+            th = (2 * np.pi * kx / nx, 2 * np.pi * ky / ny, 2 * np.pi * kz / nz)
+            f = np.cos(th[0] * i + th[1] * j + th[2] * k + ph)
+            G = 1.0 - 64.0 / np.pi ** 6 * sum(np.sin(t / 2) ** 6 for t in th)
+            assert np.abs(o.filter(f) - G * f).max() <= 2e-14, (d, kx, ky, kz)
+    assert abs((1.0 - 64.0 / np.pi ** 6) - 0.93343) < 1e-5
+
+
+def test_P15_filter_stencil_is_cubed_second_difference_and_masked_by_select():
+    """The 7-point weights (1,-6,15,-20,15,-6,1) are the second difference applied three times (binomial
+    identity), built here from np.roll; solid cells come out as +0.0 exactly, fluid cells see the solid
+    zeros like any other value."""
+    rng = np.random.default_rng(15)
+    shape = (8, 16, 8)
+    f = rng.standard_normal(shape)
+    mask = (rng.random(shape) > 0.2).astype(np.uint8)
+    d2 = lambda a, ax: np.roll(a, 1, ax) - 2 * a + np.roll(a, -1, ax)
+    ref = f + sum(d2(d2(d2(f, ax), ax), ax) for ax in range(3)) / np.pi ** 6
+    got = mk(shape, (0.1, 0.2, 0.3)).filter(f)
+    assert np.abs(got - ref).max() <= 1e-14
+    fm = np.where(mask != 0, f, 0.0)
+    refm = fm + sum(d2(d2(d2(fm, ax), ax), ax) for ax in range(3)) / np.pi ** 6
+    gotm = mk(shape, (0.1, 0.2, 0.3), mask=mask).filter(fm)
+    solid = mask == 0
+    assert np.all(gotm[solid] == 0.0) and not np.any(np.signbit(gotm[solid]))
+    assert np.abs(gotm - refm)[~solid].max() <= 1e-14
+
+
+def test_P15_filtered_step_is_step_then_filter_and_stays_solenoidal():
+    """flags bit 0: the step ends with eq. 6 on u, v, w, c (p untouched).  With beta == 1 the filter
+    commutes with the central differences, so the divergence stays at round-off."""
+    case = cases.periodic_turbulence(16, steps=1)
+    kw = dict(nu=case["nu"], alpha_c=case["alpha_c"], dt=case["dt"], n_piter=1)
+    a = mk(case["shape"], case["d"], **kw)
+    b = mk(case["shape"], case["d"], flags=1, **kw)
+    for o in (a, b):
+        o.set_fields(case["u"], case["v"], case["w"], case["c"])
+        o.step(1)
+    fa, fb = a.fields(), b.fields()
+    for k in "uvwc":
+        assert np.abs(fb[k] - a.filter(fa[k])).max() <= 1e-15 * max(1.0, np.abs(fa[k]).max())
+    assert np.array_equal(fa["p"], fb["p"])
+    div = a.div(fb["u"], fb["v"], fb["w"])
+    assert np.abs(div).max() <= 1e-12 * np.abs(fb["u"]).max() / min(case["d"])
+    # a second step runs from the filtered state (the filter output is the state)
+    b.step(1)
+    assert np.isfinite(b.fields()["u"]).all()
