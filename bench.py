@@ -48,11 +48,13 @@ def class_bytes_per_cell(masked, fb=0.0):
         "fft_z_solve": 16.0,
         "project": 56.0 + m,
         "eq9_sparse": 8.0 + m,
+        "filter": 64.0 + m,
     }
     moved = dict(canonical)
     moved["rk_stage"] = (64 + 96 + 96 + 160) / 4.0 + (1.0 if masked else 0.0)
     moved["project"] = 56.0 + (1.0 if masked else 0.0)
     moved["eq9_sparse"] = 37.0 * fb
+    moved["filter"] = 64.0 + (1.0 if masked else 0.0)
     return canonical, moved
 
 
@@ -203,7 +205,7 @@ def run_ours(args):
     N = int(np.prod(case["shape"]))
     P = case["n_piter"]
     masked = case["mask"] is not None
-    s = binding.solver_for_case(case, device=f"cuda:{local}")
+    s = binding.solver_for_case(case, device=f"cuda:{local}", flags=args.flags)
     K, W = args.steps, max(args.warmup, 3)
 
     # ---- device-resident timing: K steps, CUDA events on the solver's stream
@@ -247,7 +249,7 @@ def run_ours(args):
             f = [x.strip() for x in line.split(",")]
             if len(f) >= 3 and f[0] == dom and f[1] == case["name"]:
                 traffic = float(f[2])
-    step_bytes = canonical_bytes_per_cell(P, masked) * N
+    step_bytes = (canonical_bytes_per_cell(P, masked) + (cb["filter"] if args.flags & 1 else 0.0)) * N
     step_gbs = step_bytes / (ms_max / K * 1e-3) / 1e9
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
@@ -280,7 +282,7 @@ def run_ours(args):
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config {args.config}: {case['name']} ({N} cells), n_piter={P}, "
                                    f"{'masked room with inlet source' if masked else 'periodic box'}",
-                       "grid": list(case["shape"][::-1]), "n_piter": P,
+                       "grid": list(case["shape"][::-1]), "n_piter": P, "flags": args.flags,
                        "l2": "working set 19 fields x %.0f MB >> 126 MB L2, no flush needed" % (8 * N / 1e6),
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "gpu_launches": launches,
@@ -325,6 +327,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number (1-5)")
     ap.add_argument("--piter", type=int, default=0, help="override n_piter (0 = the config's own)")
+    ap.add_argument("--flags", type=int, default=0, help="dnslab_params_t.flags (1: eq. 6 filter, 2: per-stage projection, "
+                                                         "8: two-stage RK kernel); the headline line uses 0")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")

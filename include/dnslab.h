@@ -55,7 +55,8 @@ typedef struct {
     double dt;             /* fixed time step > 0                                                    */
     double body[3];        /* body force b (eq. 2)                                      */
     int32_t n_piter;       /* eq. 9 iterations >= 1; the paper hard-codes 4           */
-    uint32_t flags;        /* bit0 reserved (eq. 6 filter, not built); bit1: project every RK stage;
+    uint32_t flags;        /* bit0: eq. 6 filter on u,v,w,c at the end of every step (PAPER.md:84-88,
+                              central 7-point stencil, gamma = Delta^6/pi^6); bit1: project every RK stage;
                               bit2: evaluate eq. 9's right-hand side densely inside the forward x pass
                               instead of at the listed near-solid cells (same result; the library does
                               this by itself when more than half of the cells are near-solid);
@@ -124,7 +125,8 @@ int64_t dnslab_launch_count(const dnslab_t *h);
 #define DNSLAB_K_FFT_Z 4   /* fused z forward + eigenvalue division + z inverse pass       */
 #define DNSLAB_K_PROJECT 5 /* pressure-gradient projection                                 */
 #define DNSLAB_K_EQ9 6     /* eq. 9 right-hand side at the cells next to solid cells       */
-#define DNSLAB_NCLASS 7
+#define DNSLAB_K_FILTER 7  /* eq. 6 filter (flags bit 0)                                    */
+#define DNSLAB_NCLASS 8
 int dnslab_profile(dnslab_t *h, int enable);
 int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches);
 

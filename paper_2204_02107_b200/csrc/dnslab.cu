@@ -28,7 +28,7 @@ bool valid_params(const dnslab_params_t *P)
     if (P->nx < 8 || P->nx > 2048 || P->ny < 8 || P->ny > 1024 || P->nz < 8 || P->nz > 1024) return false;
     if (!(P->dx > 0) || !(P->dy > 0) || !(P->dz > 0) || !(P->dt > 0)) return false;
     if (!(P->nu >= 0) || !(P->alpha_c >= 0) || P->n_piter < 1) return false;
-    if (P->flags & ~14u) return false;
+    if (P->flags & ~15u) return false;
     return true;
 }
 
@@ -468,6 +468,31 @@ int launch_eq9_sparse(dnslab *h, const double *p, bool first)
     return check_launch(h);
 }
 
+// NEXT-1: eq. 6 filter of the four fields, in -> out (different buffers)
+int launch_filter(dnslab *h, double *const *in, double *const *out)
+{
+    dnsst::FilterArgs a;
+    for (int m = 0; m < 4; ++m) {
+        a.in[m] = in[m];
+        a.out[m] = out[m];
+    }
+    a.face = h->face;
+    a.nx = h->P.nx; a.ny = h->P.ny; a.nz = h->P.nz;
+    const double pi = 3.14159265358979323846;
+    a.g = 1.0 / (pi * pi * pi * pi * pi * pi);
+    const dim3 blk(h->P.nx < 32 ? h->P.nx : 32, h->P.ny < 8 ? h->P.ny : 8, 1);
+    // enough blocks for >= 4 waves of 8 blocks per SM, at least 8 planes per block
+    const long tiles = 4L * (h->P.nx / blk.x) * (h->P.ny / blk.y);
+    int kc = h->P.nz;
+    while (kc > 8 && tiles * (h->P.nz / kc) < 32L * h->nsm) kc /= 2;
+    a.kc = kc;
+    const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, 4 * (h->P.nz / kc));
+    ProfScope ps(h, DNSLAB_K_FILTER);
+    if (h->face) dnsst::k_filter<true><<<grd, blk, 0, h->stream>>>(a);
+    else dnsst::k_filter<false><<<grd, blk, 0, h->stream>>>(a);
+    return check_launch(h);
+}
+
 // divergence, n_piter iterations of eq. 9 warm-started from p, correction (in place on q)
 int pressure_stage(dnslab *h, double *const *q, double *p)
 {
@@ -693,7 +718,7 @@ int dnslab_set_fields(dnslab_t *h, const double *u, const double *v, const doubl
 int dnslab_step(dnslab_t *h, int32_t nsteps)
 {
     if (!h || nsteps < 0) return DNSLAB_EINVAL;
-    const bool stage_proj = (h->P.flags & 2u) != 0;
+    const bool stage_proj = (h->P.flags & 2u) != 0, filter = (h->P.flags & 1u) != 0;
     const size_t bytes = h->n * sizeof(double);
     int rc;
     for (int it = 0; it < nsteps; ++it) {
@@ -710,10 +735,16 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
         }
         if (!stage_proj) {
             if ((rc = pressure_stage(h, h->A, h->p))) return rc;
+            // new state: A, or (flags bit 0) its filtered copy in Qc, which this path does not use otherwise
+            double **fin = h->A;
+            if (filter) {
+                if ((rc = launch_filter(h, h->A, h->Qc))) return rc;
+                fin = h->Qc;
+            }
             for (int m = 0; m < 4; ++m) {
                 double *t = h->Q[m];
-                h->Q[m] = h->A[m];
-                h->A[m] = t;
+                h->Q[m] = fin[m];
+                fin[m] = t;
             }
             continue;
         }
@@ -729,10 +760,15 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
         if ((rc = pressure_stage(h, h->A, h->ps))) return rc;
         if ((rc = launch_rk<4, false>(h, h->A, nullptr, nullptr, nullptr))) return rc;
         if ((rc = pressure_stage(h, h->Qc, h->p))) return rc;
+        double **fin = h->Qc;
+        if (filter) {
+            if ((rc = launch_filter(h, h->Qc, h->A))) return rc;
+            fin = h->A;
+        }
         for (int m = 0; m < 4; ++m) {
             double *t = h->Q[m];
-            h->Q[m] = h->Qc[m];
-            h->Qc[m] = t;
+            h->Q[m] = fin[m];
+            fin[m] = t;
         }
     }
     return DNSLAB_OK;

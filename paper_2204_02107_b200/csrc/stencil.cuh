@@ -866,6 +866,57 @@ __global__ void __launch_bounds__(256) k_eq9_sparse(double *__restrict__ d, cons
     d[o] = dv + ((gxp - gxm) * r2x + (gyp - gym) * r2y + (gzp - gzm) * r2z);
 }
 
+// NEXT-1, eq. 6: out = beta ? f + sum_a gamma_a d6_a f : +0.0 with gamma_a = Delta_a^6/pi^6 and
+// d6_a the central 7-point stencil (1,-6,15,-20,15,-6,1)/Delta_a^6 (reading R23), on u, v, w, c.
+// One thread per (x, y) column of one field, marching kc planes: the seven z values ride in registers,
+// the x and y neighbours come through L1 (a block touches a 38 x 14 patch of each plane).
+// blockIdx.z enumerates (z chunk, field).
+struct FilterArgs {
+    const double *in[4];
+    double *out[4];
+    const uint8_t *face; // null: no solid cells
+    int nx, ny, nz, kc;
+    double g;            // 1/pi^6
+};
+
+template <bool MASKED> __global__ void __launch_bounds__(256) k_filter(const FilterArgs a)
+{
+    const int nx = a.nx, ny = a.ny, nz = a.nz;
+    const int m = blockIdx.z & 3, k0 = (blockIdx.z >> 2) * a.kc;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+    const double *__restrict__ f = a.in[m];
+    double *__restrict__ o = a.out[m];
+    const size_t plane = (size_t)nx * ny;
+    const size_t col = (size_t)nx * j + i, row = (size_t)nx * j;
+    size_t xo[6], yo[6];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        xo[d] = row + ((i - 3 + d) & (nx - 1));
+        xo[3 + d] = row + ((i + 1 + d) & (nx - 1));
+        yo[d] = (size_t)nx * ((j - 3 + d) & (ny - 1)) + i;
+        yo[3 + d] = (size_t)nx * ((j + 1 + d) & (ny - 1)) + i;
+    }
+    double z[7]; // z[3] is the centre
+#pragma unroll
+    for (int d = 0; d < 6; ++d) z[d + 1] = __ldg(f + plane * (size_t)((k0 - 3 + d) & (nz - 1)) + col);
+    for (int t = 0; t < a.kc; ++t) {
+        const int k = k0 + t;
+        const size_t pk = plane * (size_t)k;
+#pragma unroll
+        for (int d = 0; d < 6; ++d) z[d] = z[d + 1];
+        z[6] = __ldg(f + plane * (size_t)((k + 3) & (nz - 1)) + col);
+        bool fluid = true;
+        if (MASKED) fluid = (a.face[pk + col] & 1) != 0;
+        const double f0 = z[3];
+        const double sx = __ldg(f + pk + xo[0]) - 6.0 * __ldg(f + pk + xo[1]) + 15.0 * __ldg(f + pk + xo[2]) - 20.0 * f0 +
+                          15.0 * __ldg(f + pk + xo[3]) - 6.0 * __ldg(f + pk + xo[4]) + __ldg(f + pk + xo[5]);
+        const double sy = __ldg(f + pk + yo[0]) - 6.0 * __ldg(f + pk + yo[1]) + 15.0 * __ldg(f + pk + yo[2]) - 20.0 * f0 +
+                          15.0 * __ldg(f + pk + yo[3]) - 6.0 * __ldg(f + pk + yo[4]) + __ldg(f + pk + yo[5]);
+        const double sz = z[0] - 6.0 * z[1] + 15.0 * z[2] - 20.0 * f0 + 15.0 * z[4] - 6.0 * z[5] + z[6];
+        o[pk + col] = fluid ? f0 + a.g * ((sx + sy) + sz) : 0.0;
+    }
+}
+
 // a6: u_a = beta ? u*_a - delta_a p : +0.0, in place (eq. 8)
 template <bool MASKED>
 __global__ void __launch_bounds__(256) k_project(double *__restrict__ u, double *__restrict__ v, double *__restrict__ w, const double *__restrict__ p,

@@ -32,7 +32,7 @@ def compare(got, ref, tol, mask=None, what=""):
 
 def run_both(case, checkpoints, n_piter=None, flags=0):
     s = binding.solver_for_case(case, n_piter=n_piter, flags=flags)
-    o = oracle_for(case, n_piter=n_piter, flags=flags & 2)   # only bit 1 changes the method; the rest pick kernels
+    o = oracle_for(case, n_piter=n_piter, flags=flags & 3)   # bits 0 and 1 change the method; the rest pick kernels
     done = 0
     for cp in checkpoints:
         s.step(cp - done)
@@ -136,6 +136,22 @@ def test_per_stage_projection_variant():
     case = cases.duct_room(32, 16, 16)
     for cp, got, ref in run_both(case, [1, 5], flags=2):
         compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"flags=2 step {cp}")
+
+
+def test_eq6_filter_variant():
+    """NEXT-1, flags bit 0: eq. 6 filter on u, v, w, c at the end of every step (masked room with sources, periodic
+    box, with per-stage projection, with the two-stage RK kernel, and a grid thinner than the stencil is wide)."""
+    for case, cps, flags in [(cases.duct_room(64, 32, 32), [1, 20], 1), (cases.periodic_turbulence(32, steps=5), [1, 5], 1),
+                             (cases.duct_room(32, 16, 16), [1, 5], 3), (cases.duct_room(64, 32, 32), [1, 5], 9),
+                             (cases.duct_room(32, 8, 8), [1, 3], 1)]:
+        for cp, got, ref in run_both(case, cps, flags=flags):
+            compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"flags={flags} {case['name']} step {cp}")
+    case = cases.duct_room(64, 32, 32)
+    s = binding.solver_for_case(case, flags=1)
+    n0 = s.launch_count()
+    s.step(1)
+    assert s.launch_count() - n0 == 4 + 1 + 4 * 6 + 1 + 1
+    s.close()
 
 
 def test_two_stage_rk_kernel_variant():
