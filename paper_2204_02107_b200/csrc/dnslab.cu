@@ -480,6 +480,25 @@ int launch_filter(dnslab *h, double *const *in, double *const *out)
     a.nx = h->P.nx; a.ny = h->P.ny; a.nz = h->P.nz;
     const double pi = 3.14159265358979323846;
     a.g = 1.0 / (pi * pi * pi * pi * pi * pi);
+    ProfScope ps(h, DNSLAB_K_FILTER);
+    if (h->P.nx >= dnsst::FM_TX && h->P.ny >= dnsst::FM_TY && !getenv("DNSLAB_FILTER_SIMPLE")) {
+        // z-marching kernel: 64 x 8 columns of one field; >= 4 waves of 4 blocks per SM, at least 8 planes per block
+        const long tiles = 4L * (h->P.nx / dnsst::FM_TX) * (h->P.ny / dnsst::FM_TY);
+        int kc = h->P.nz;
+        while (kc > 8 && tiles * (h->P.nz / kc) < 16L * h->nsm) kc /= 2;
+        a.kc = kc;
+        const dim3 blk(32, dnsst::FM_TY, 1);
+        const dim3 grd(h->P.nx / dnsst::FM_TX, h->P.ny / dnsst::FM_TY, 4 * (h->P.nz / kc));
+        const size_t smem = dnsst::FM_SMEM;
+        if (h->face) {
+            CK(cudaFuncSetAttribute(dnsst::k_filter_march<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            dnsst::k_filter_march<true><<<grd, blk, smem, h->stream>>>(a);
+        } else {
+            CK(cudaFuncSetAttribute(dnsst::k_filter_march<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            dnsst::k_filter_march<false><<<grd, blk, smem, h->stream>>>(a);
+        }
+        return check_launch(h);
+    }
     const dim3 blk(h->P.nx < 32 ? h->P.nx : 32, h->P.ny < 8 ? h->P.ny : 8, 1);
     // enough blocks for >= 4 waves of 8 blocks per SM, at least 8 planes per block
     const long tiles = 4L * (h->P.nx / blk.x) * (h->P.ny / blk.y);
@@ -487,7 +506,6 @@ int launch_filter(dnslab *h, double *const *in, double *const *out)
     while (kc > 8 && tiles * (h->P.nz / kc) < 32L * h->nsm) kc /= 2;
     a.kc = kc;
     const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, 4 * (h->P.nz / kc));
-    ProfScope ps(h, DNSLAB_K_FILTER);
     if (h->face) dnsst::k_filter<true><<<grd, blk, 0, h->stream>>>(a);
     else dnsst::k_filter<false><<<grd, blk, 0, h->stream>>>(a);
     return check_launch(h);

@@ -917,6 +917,92 @@ template <bool MASKED> __global__ void __launch_bounds__(256) k_filter(const Fil
     }
 }
 
+// k_filter_march: eq. 6 for grids with nx >= 64, ny >= 8.  A block owns a 64 x 8 (x by y) column of ONE field
+// and walks kc planes; each thread owns two x-adjacent cells.  Plane tiles (14 rows x 72 doubles: three-cell
+// halo in y, four in x so that every pair is 16-byte aligned) arrive by cp.async, two planes in flight; the
+// x and y neighbours of plane k come from its tile, the z+3 value from the tile of plane k+3, the other six
+// z values ride in registers.  Every value is fetched from L2/HBM once per block (plus halo).
+constexpr int FM_TX = 64, FM_TY = 8, FM_W = FM_TX + 8, FM_ROWS = FM_TY + 6, FM_NBUF = 6;
+constexpr int FM_TILE = FM_ROWS * FM_W;
+constexpr int FM_SMEM = FM_NBUF * FM_TILE * (int)sizeof(double);
+constexpr int FM_CHUNKS = FM_ROWS * (FM_W / 2);
+
+template <bool MASKED> __global__ void __launch_bounds__(256) k_filter_march(const FilterArgs a)
+{
+    extern __shared__ double2 fm_smem2[];
+    double *sm = reinterpret_cast<double *>(fm_smem2);
+    const int nx = a.nx, ny = a.ny, nz = a.nz, kc = a.kc;
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * 32 + tx;
+    const int m = blockIdx.z & 3, k0 = (blockIdx.z >> 2) * kc;
+    const int x0 = blockIdx.x * FM_TX, y0 = blockIdx.y * FM_TY;
+    const double *__restrict__ f = a.in[m];
+    double *__restrict__ o = a.out[m];
+    const size_t plane = (size_t)nx * ny;
+    const size_t col = (size_t)nx * (y0 + ty) + x0 + 2 * tx;
+    const int own = (ty + 3) * FM_W + 4 + 2 * tx;
+
+    // this thread's chunks of one plane tile
+    const int c1 = tid + 256;
+    const int r0 = tid / (FM_W / 2), q0 = tid - r0 * (FM_W / 2), r1 = c1 / (FM_W / 2), q1 = c1 - r1 * (FM_W / 2);
+    const bool has1 = c1 < FM_CHUNKS;
+    const unsigned s0 = (unsigned)nx * ((y0 - 3 + r0) & (ny - 1)) + ((x0 - 4 + 2 * q0) & (nx - 1));
+    const unsigned s1 = (unsigned)nx * ((y0 - 3 + r1) & (ny - 1)) + ((x0 - 4 + 2 * q1) & (nx - 1));
+    const int d0 = r0 * FM_W + 2 * q0, d1 = r1 * FM_W + 2 * q1;
+    auto issue = [&](int n) { // plane k0+n into tile n % 6
+        const double *src = f + plane * (size_t)((k0 + n) & (nz - 1));
+        double *dst = sm + (n % FM_NBUF) * FM_TILE;
+        cp_async16(dst + d0, src + s0);
+        if (has1) cp_async16(dst + d1, src + s1);
+    };
+#pragma unroll
+    for (int n = 0; n < 5; ++n) {
+        issue(n);
+        cp_async_commit();
+    }
+    double2 z[7]; // z[3] is the centre plane
+#pragma unroll
+    for (int d = 0; d < 3; ++d) z[d + 1] = __ldg(reinterpret_cast<const double2 *>(f + plane * (size_t)((k0 - 3 + d) & (nz - 1)) + col));
+    asm volatile("cp.async.wait_group 2;\n" ::: "memory");
+    __syncthreads();
+#pragma unroll
+    for (int d = 0; d < 3; ++d) z[d + 4] = *reinterpret_cast<const double2 *>(sm + d * FM_TILE + own);
+
+    for (int t = 0; t < kc; ++t) {
+        const size_t pk = plane * (size_t)(k0 + t);
+        unsigned fA = 1, fB = 1;
+        if (MASKED) {
+            const uchar2 fv = *reinterpret_cast<const uchar2 *>(a.face + pk + col);
+            fA = fv.x;
+            fB = fv.y;
+        }
+        cp_async_wait_one();
+        __syncthreads(); // tile t+3 visible; every thread is done with tile t-1
+        if (t + 5 <= kc + 2) issue(t + 5);
+        cp_async_commit();
+#pragma unroll
+        for (int d = 0; d < 6; ++d) z[d] = z[d + 1];
+        z[6] = *reinterpret_cast<const double2 *>(sm + ((t + 3) % FM_NBUF) * FM_TILE + own);
+        const double *sc = sm + (t % FM_NBUF) * FM_TILE + own;
+        const double2 xa = *reinterpret_cast<const double2 *>(sc - 4), xb = *reinterpret_cast<const double2 *>(sc - 2);
+        const double2 xc = *reinterpret_cast<const double2 *>(sc + 2), xd = *reinterpret_cast<const double2 *>(sc + 4);
+        const double2 c = z[3];
+        // cell A = c.x: x-3..x+3 = xa.y xb.x xb.y | c.y xc.x xc.y;   cell B = c.y: xb.x xb.y c.x | xc.x xc.y xd.x
+        const double sxA = xa.y - 6.0 * xb.x + 15.0 * xb.y - 20.0 * c.x + 15.0 * c.y - 6.0 * xc.x + xc.y;
+        const double sxB = xb.x - 6.0 * xb.y + 15.0 * c.x - 20.0 * c.y + 15.0 * xc.x - 6.0 * xc.y + xd.x;
+        const double2 y0v = *reinterpret_cast<const double2 *>(sc - 3 * FM_W), y1v = *reinterpret_cast<const double2 *>(sc - 2 * FM_W);
+        const double2 y2v = *reinterpret_cast<const double2 *>(sc - FM_W), y4v = *reinterpret_cast<const double2 *>(sc + FM_W);
+        const double2 y5v = *reinterpret_cast<const double2 *>(sc + 2 * FM_W), y6v = *reinterpret_cast<const double2 *>(sc + 3 * FM_W);
+        const double syA = y0v.x - 6.0 * y1v.x + 15.0 * y2v.x - 20.0 * c.x + 15.0 * y4v.x - 6.0 * y5v.x + y6v.x;
+        const double syB = y0v.y - 6.0 * y1v.y + 15.0 * y2v.y - 20.0 * c.y + 15.0 * y4v.y - 6.0 * y5v.y + y6v.y;
+        const double szA = z[0].x - 6.0 * z[1].x + 15.0 * z[2].x - 20.0 * c.x + 15.0 * z[4].x - 6.0 * z[5].x + z[6].x;
+        const double szB = z[0].y - 6.0 * z[1].y + 15.0 * z[2].y - 20.0 * c.y + 15.0 * z[4].y - 6.0 * z[5].y + z[6].y;
+        double2 r;
+        r.x = (!MASKED || (fA & 1)) ? c.x + a.g * ((sxA + syA) + szA) : 0.0;
+        r.y = (!MASKED || (fB & 1)) ? c.y + a.g * ((sxB + syB) + szB) : 0.0;
+        *reinterpret_cast<double2 *>(o + pk + col) = r;
+    }
+}
+
 // a6: u_a = beta ? u*_a - delta_a p : +0.0, in place (eq. 8)
 template <bool MASKED>
 __global__ void __launch_bounds__(256) k_project(double *__restrict__ u, double *__restrict__ v, double *__restrict__ w, const double *__restrict__ p,
