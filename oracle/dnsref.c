@@ -443,6 +443,69 @@ int dnsref_step(dnsref_t *h, int nsteps)
     return DNSREF_OK;
 }
 
+/* ------------------------------------------------------------------------
+ * NEXT-3: the two global reductions the paper's main loop uses.
+ *
+ * Courant number of the current state ("the user also specifies the maximum Courant number, as
+ * the implementation utilizes dynamic time stepping (in AdjustDt.m)"); the formula is not printed -- reading R24:
+ *     Co = dt * max over all cells of ( |u|/dx + |v|/dy + |w|/dz ).
+ * The caller turns it into the next dt (dt_new = Co_max / (Co/dt)) and sets it with dnsref_set_dt.
+ * ---------------------------------------------------------------------- */
+double dnsref_courant(const dnsref_t *h)
+{
+    double best = 0.0;
+    for (int64_t o = 0; o < h->n; ++o) {
+        const double r = fabs(h->q[0][o]) / h->P.dx + fabs(h->q[1][o]) / h->P.dy + fabs(h->q[2][o]) / h->P.dz;
+        if (r > best) best = r;
+    }
+    return best * h->P.dt;
+}
+
+int dnsref_set_dt(dnsref_t *h, double dt)
+{
+    if (!h || !(dt > 0)) return DNSREF_EINVAL;
+    h->P.dt = dt;
+    return DNSREF_OK;
+}
+
+/* Mean and standard deviation of the scalar over the fluid cells of an index box that wraps modulo N
+ * ("the mean CO2 content as a function of simulation time ... The standard deviation is
+ * plotted as well") -- reading R25: population standard deviation sqrt(sum (c - mean)^2 / count) over the
+ * cells with beta = 1 inside the box; two passes, plain index-order sums.  out[0] = mean, out[1] = std,
+ * out[2] = count.  A box without fluid cells gives 0, 0, 0. */
+int dnsref_scalar_stats(const dnsref_t *h, const int32_t lo[3], const int32_t size[3], double out[3])
+{
+    if (!h || !lo || !size || !out) return DNSREF_EINVAL;
+    const int nx = h->P.nx, ny = h->P.ny, nz = h->P.nz;
+    if (size[0] < 1 || size[1] < 1 || size[2] < 1 || size[0] > nx || size[1] > ny || size[2] > nz) return DNSREF_EINVAL;
+    double sum = 0.0;
+    int64_t cnt = 0;
+    for (int k = 0; k < size[2]; ++k)
+        for (int j = 0; j < size[1]; ++j)
+            for (int i = 0; i < size[0]; ++i) {
+                const int64_t o = IDX(wrapm(lo[0] + i, nx), wrapm(lo[1] + j, ny), wrapm(lo[2] + k, nz));
+                if (!h->beta[o]) continue;
+                sum += h->q[3][o];
+                ++cnt;
+            }
+    out[0] = out[1] = 0.0;
+    out[2] = (double)cnt;
+    if (cnt == 0) return DNSREF_OK;
+    const double mean = sum / (double)cnt;
+    double ss = 0.0;
+    for (int k = 0; k < size[2]; ++k)
+        for (int j = 0; j < size[1]; ++j)
+            for (int i = 0; i < size[0]; ++i) {
+                const int64_t o = IDX(wrapm(lo[0] + i, nx), wrapm(lo[1] + j, ny), wrapm(lo[2] + k, nz));
+                if (!h->beta[o]) continue;
+                const double dv = h->q[3][o] - mean;
+                ss += dv * dv;
+            }
+    out[0] = mean;
+    out[1] = sqrt(ss / (double)cnt);
+    return DNSREF_OK;
+}
+
 /* ------------------------------------------------------------------------ */
 static int valid_params(const dnsref_params_t *P)
 {

@@ -57,6 +57,10 @@ def lib():
         L.dnsref_div.restype = None
         L.dnsref_poisson_rhs.argtypes = [C.c_void_p] + [C.c_void_p] * 3
         L.dnsref_poisson_rhs.restype = None
+        L.dnsref_courant.argtypes = [C.c_void_p]
+        L.dnsref_courant.restype = C.c_double
+        L.dnsref_set_dt.argtypes = [C.c_void_p, C.c_double]
+        L.dnsref_scalar_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_double)]
         L.dnsref_filter.argtypes = [C.c_void_p] + [C.c_void_p] * 2
         L.dnsref_filter.restype = None
         L.dnsref_project.argtypes = [C.c_void_p] + [C.c_void_p] * 7
@@ -181,6 +185,26 @@ class Oracle:
         r = self._new()
         lib().dnsref_poisson_rhs(self._h, _ptr(d), _ptr(p), _ptr(r))
         return r
+
+    def courant(self):
+        """dt * max_cells(|u|/dx + |v|/dy + |w|/dz) of the current state (reading R24)."""
+        return float(lib().dnsref_courant(self._h))
+
+    def set_dt(self, dt):
+        rc = lib().dnsref_set_dt(self._h, float(dt))
+        if rc:
+            raise ValueError("dnsref_set_dt")
+        self.P.dt = float(dt)
+
+    def scalar_stats(self, lo, size):
+        """(mean, std, count) of c over the fluid cells of the index box lo (x,y,z), size (x,y,z) (reading R25)."""
+        a = (C.c_int32 * 3)(*[int(x) for x in lo])
+        b = (C.c_int32 * 3)(*[int(x) for x in size])
+        out = (C.c_double * 3)()
+        rc = lib().dnsref_scalar_stats(self._h, a, b, out)
+        if rc:
+            raise ValueError("dnsref_scalar_stats")
+        return out[0], out[1], int(out[2])
 
     def filter(self, f):
         """eq. 6 on one field (masked by the select)."""

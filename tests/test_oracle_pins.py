@@ -525,3 +525,67 @@ def test_P15_filtered_step_is_step_then_filter_and_stays_solenoidal():
     # a second step runs from the filtered state (the filter output is the state)
     b.step(1)
     assert np.isfinite(b.fields()["u"]).all()
+
+
+# ---------------------------------------------------------------- reductions (P16, NEXT-3)
+def test_P16_courant_number_closed_forms():
+    """Co = dt max(|u|/dx + |v|/dy + |w|/dz): exact for a uniform field, picks out a single spike wherever it
+    sits (incl. the last cell), scales with dt, ignores the sign."""
+    shape, d = (8, 16, 32), (0.1, 0.2, 0.25)
+    o = mk(shape, d, dt=0.5)
+    one = np.ones(shape)
+    o.set_fields(0.3 * one, -0.4 * one, 0.5 * one, 0 * one)
+    assert o.courant() == 0.5 * (0.3 / 0.1 + 0.4 / 0.2 + 0.5 / 0.25)
+    for pos in [(0, 0, 0), (7, 15, 31), (3, 9, 17)]:
+        u = 0.3 * one
+        u[pos] = -2.0
+        o.set_fields(u, -0.4 * one, 0.5 * one, 0 * one)
+        assert o.courant() == 0.5 * (2.0 / 0.1 + 0.4 / 0.2 + 0.5 / 0.25)
+    o.set_dt(0.25)
+    assert o.courant() == 0.25 * (2.0 / 0.1 + 0.4 / 0.2 + 0.5 / 0.25)
+    # the step uses the new dt: shear-flow decay factor of P7 with dt = 0.25
+    with pytest.raises(ValueError):
+        o.set_dt(0.0)
+
+
+def test_P16_set_dt_changes_the_step():
+    """Two steps of dt/2 set through set_dt equal two steps of an oracle created with dt/2, and differ from dt."""
+    case = cases.taylor_green(16)
+    kw = dict(nu=case["nu"], alpha_c=case["alpha_c"], n_piter=1)
+    a = mk(case["shape"], case["d"], dt=case["dt"], **kw)
+    b = mk(case["shape"], case["d"], dt=case["dt"] / 2, **kw)
+    for o in (a, b):
+        o.set_fields(case["u"], case["v"], case["w"], case["c"])
+    a.set_dt(case["dt"] / 2)
+    a.step(2)
+    b.step(2)
+    assert all(np.array_equal(a.fields()[k], b.fields()[k]) for k in "uvwcp")
+
+
+def test_P16_scalar_stats_closed_form_library_and_mask():
+    """Mean/std of c over the fluid cells of a wrapping box: a full-box cosine mode has mean 0 and std 1/sqrt 2;
+    numpy's own mean/std (pairwise sums, a different routine) agree on a random field with a random mask and a
+    box that wraps through the periodic seam; solid cells are left out; an all-solid box gives (0, 0, 0)."""
+    shape = (8, 16, 32)
+    nz, ny, nx = shape
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    o = mk(shape)
+    z = np.zeros(shape)
+    o.set_fields(z, z, z, 3.0 + np.cos(2 * np.pi * 3 * i / nx + 0.4))
+    m, s, n = o.scalar_stats((0, 0, 0), (nx, ny, nz))
+    assert n == nx * ny * nz and abs(m - 3.0) < 1e-13 and abs(s - math.sqrt(0.5)) < 1e-13   # plain index-order sums of 4096 terms
+    r = np.random.default_rng(16)
+    c = r.standard_normal(shape)
+    mask = (r.random(shape) > 0.3).astype(np.uint8)
+    o = mk(shape, mask=mask)
+    o.set_fields(z, z, z, c)
+    lo, size = (28, 10, 6), (9, 11, 5)          # wraps in x, y and z
+    sel = np.zeros(shape, bool)
+    sel[np.ix_([(lo[2] + a) % nz for a in range(size[2])], [(lo[1] + a) % ny for a in range(size[1])],
+               [(lo[0] + a) % nx for a in range(size[0])])] = True
+    sel &= mask != 0
+    m, s, n = o.scalar_stats(lo, size)
+    assert n == sel.sum() and abs(m - c[sel].mean()) < 1e-14 and abs(s - c[sel].std()) < 1e-14
+    solid = mk(shape, mask=np.zeros(shape, np.uint8))
+    solid.set_fields(z, z, z, c)
+    assert solid.scalar_stats((0, 0, 0), (4, 4, 4)) == (0.0, 0.0, 0)
