@@ -126,9 +126,25 @@ int64_t dnslab_launch_count(const dnslab_t *h);
 #define DNSLAB_K_PROJECT 5 /* pressure-gradient projection                                 */
 #define DNSLAB_K_EQ9 6     /* eq. 9 right-hand side at the cells next to solid cells       */
 #define DNSLAB_K_FILTER 7  /* eq. 6 filter (flags bit 0)                                    */
-#define DNSLAB_NCLASS 8
+#define DNSLAB_K_REDUCE 8  /* Courant-number and scalar mean/std reductions (NEXT-3)         */
+#define DNSLAB_NCLASS 9
 int dnslab_profile(dnslab_t *h, int enable);
 int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches);
+
+/* ---- NEXT-3: the reductions of the paper's main loop --------------------------------------------------
+ * dnslab_courant: Co = dt * max over all cells of (|u|/dx + |v|/dy + |w|/dz) of the current state -- the
+ * quantity the paper's dynamic time stepping limits ("AdjustDt.m"; formula not printed, DESIGN.md
+ * reading R24).  *co is HOST memory; the call synchronises the stream.  Bit-identical to a plain loop.
+ * dnslab_set_dt: the time step used by the following dnslab_step calls (dt > 0, else DNSLAB_EINVAL); the
+ * caller's control law is dt_new = Co_max * dt / Co.
+ * dnslab_scalar_stats: mean, population standard deviation and count of the scalar c over the FLUID cells of the
+ * index box lo[0..2] (x,y,z), size[0..2] (1 <= size[a] <= N_a; the box wraps modulo N) -- the "mean CO2
+ * content" and its standard deviation monitored in PAPER.md:265-269 (reading R25).  out[0..2] is HOST memory
+ * (mean, std, count); a box without fluid cells gives zeros.  Synchronises the stream.  Partial sums are combined
+ * in a fixed order (reproducible), which is not the order of a plain loop: agreement to ~1e-13 relative. */
+int dnslab_courant(dnslab_t *h, double *co);
+int dnslab_set_dt(dnslab_t *h, double dt);
+int dnslab_scalar_stats(dnslab_t *h, const int32_t lo[3], const int32_t size[3], double out[3]);
 
 int dnslab_destroy(dnslab_t *h);
 

@@ -12,8 +12,8 @@ LIB_PATH = os.path.join(_HERE, "libdnslab.so")
 
 SYMBOLS = ["dnslab_workspace_bytes", "dnslab_create", "dnslab_set_fields", "dnslab_step", "dnslab_poisson",
            "dnslab_fields", "dnslab_get_fields", "dnslab_launch_count", "dnslab_profile", "dnslab_profile_read",
-           "dnslab_destroy", "dnslab_strerror"]
-KERNEL_CLASSES = ["rk_stage", "div", "fft_x", "fft_y", "fft_z_solve", "project", "eq9_sparse", "filter"]
+           "dnslab_courant", "dnslab_set_dt", "dnslab_scalar_stats", "dnslab_destroy", "dnslab_strerror"]
+KERNEL_CLASSES = ["rk_stage", "div", "fft_x", "fft_y", "fft_z_solve", "project", "eq9_sparse", "filter", "reduce"]
 
 
 class Params(C.Structure):
@@ -57,6 +57,9 @@ def lib():
         L.dnslab_launch_count.restype = C.c_int64
         L.dnslab_profile.argtypes = [C.c_void_p, C.c_int]
         L.dnslab_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        L.dnslab_courant.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.dnslab_set_dt.argtypes = [C.c_void_p, C.c_double]
+        L.dnslab_scalar_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_double)]
         L.dnslab_destroy.argtypes = [C.c_void_p]
         L.dnslab_strerror.argtypes = [C.c_int]
         L.dnslab_strerror.restype = C.c_char_p
@@ -167,6 +170,23 @@ class Solver:
 
     def launch_count(self):
         return int(lib().dnslab_launch_count(self._h))
+
+    def courant(self):
+        """dnslab_courant: dt * max_cells(|u|/dx + |v|/dy + |w|/dz); synchronises."""
+        out = C.c_double(0.0)
+        _check(lib().dnslab_courant(self._h, C.byref(out)), "dnslab_courant")
+        return out.value
+
+    def set_dt(self, dt):
+        _check(lib().dnslab_set_dt(self._h, float(dt)), "dnslab_set_dt")
+
+    def scalar_stats(self, lo, size):
+        """dnslab_scalar_stats: (mean, std, count) of c over the fluid cells of the index box lo, size (x,y,z)."""
+        a = (C.c_int32 * 3)(*[int(x) for x in lo])
+        b = (C.c_int32 * 3)(*[int(x) for x in size])
+        out = (C.c_double * 3)()
+        _check(lib().dnslab_scalar_stats(self._h, a, b, out), "dnslab_scalar_stats")
+        return out[0], out[1], int(out[2])
 
     def profile(self, enable):
         _check(lib().dnslab_profile(self._h, int(bool(enable))), "dnslab_profile")

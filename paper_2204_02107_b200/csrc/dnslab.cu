@@ -11,6 +11,7 @@
 
 #include "../../include/dnslab.h"
 #include "fft.cuh"
+#include "reduce.cuh"
 #include "stencil.cuh"
 
 using dnsfft::c2;
@@ -845,6 +846,73 @@ int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches)
         ms[c] = h->prof_ms[c];
         launches[c] = h->prof_n[c];
     }
+    return DNSLAB_OK;
+}
+
+int dnslab_courant(dnslab_t *h, double *co)
+{
+    if (!h || !co) return DNSLAB_EINVAL;
+    unsigned long long *res = reinterpret_cast<unsigned long long *>(h->W); // W is scratch outside a solve
+    CK(cudaMemsetAsync(res, 0, sizeof(*res), h->stream));
+    {
+        ProfScope ps(h, DNSLAB_K_REDUCE);
+        size_t g = (h->n + 255) / 256;
+        if (g > (size_t)16 * h->nsm) g = (size_t)16 * h->nsm;
+        dnsred::k_courant<<<(unsigned)g, 256, 0, h->stream>>>(h->Q[0], h->Q[1], h->Q[2], h->n, h->P.dx, h->P.dy, h->P.dz, res);
+        if (int rc = check_launch(h)) return rc;
+    }
+    double rate = 0.0;
+    CK(cudaMemcpyAsync(&rate, res, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    *co = rate * h->P.dt;
+    return DNSLAB_OK;
+}
+
+int dnslab_set_dt(dnslab_t *h, double dt)
+{
+    if (!h || !(dt > 0)) return DNSLAB_EINVAL;
+    h->P.dt = dt;
+    return DNSLAB_OK;
+}
+
+int dnslab_scalar_stats(dnslab_t *h, const int32_t lo[3], const int32_t size[3], double out[3])
+{
+    if (!h || !lo || !size || !out) return DNSLAB_EINVAL;
+    const int nn[3] = {h->P.nx, h->P.ny, h->P.nz};
+    dnsred::BoxArgs a;
+    a.c = h->Q[3];
+    a.face = h->face;
+    a.nx = nn[0]; a.ny = nn[1]; a.nz = nn[2];
+    a.count = 1;
+    for (int d = 0; d < 3; ++d) {
+        if (size[d] < 1 || size[d] > nn[d]) return DNSLAB_EINVAL;
+        a.lo[d] = ((lo[d] % nn[d]) + nn[d]) % nn[d];
+        a.size[d] = size[d];
+        a.count *= (size_t)size[d];
+    }
+    // W (scratch outside a solve): res[0..3], then 2 G partials
+    double *res = h->W, *part = h->W + 8;
+    size_t G = (a.count + 4095) / 4096;
+    const size_t gmax = (size_t)8 * h->nsm < (h->n - 8) / 2 ? (size_t)8 * h->nsm : (h->n - 8) / 2;
+    if (G > gmax) G = gmax;
+    if (G < 1) G = 1;
+    const size_t chunk = (a.count + G - 1) / G;
+    {
+        ProfScope ps(h, DNSLAB_K_REDUCE);
+        dnsred::k_box_partial<0><<<(unsigned)G, 256, 0, h->stream>>>(a, chunk, res, part);
+        if (int rc = check_launch(h)) return rc;
+    }
+    dnsred::k_box_final<0><<<1, 256, 0, h->stream>>>(part, (int)G, res);
+    if (int rc = check_launch(h)) return rc;
+    {
+        ProfScope ps(h, DNSLAB_K_REDUCE);
+        dnsred::k_box_partial<1><<<(unsigned)G, 256, 0, h->stream>>>(a, chunk, res, part);
+        if (int rc = check_launch(h)) return rc;
+    }
+    dnsred::k_box_final<1><<<1, 256, 0, h->stream>>>(part, (int)G, res);
+    if (int rc = check_launch(h)) return rc;
+    CK(cudaMemcpyAsync(out, res, 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
     return DNSLAB_OK;
 }
 

@@ -154,6 +154,44 @@ def test_eq6_filter_variant():
     s.close()
 
 
+def test_next3_courant_set_dt_and_scalar_stats():
+    """NEXT-3: the Courant number is bit-identical to the oracle's plain loop; set_dt changes the following steps
+    on both sides alike (a Courant-limited run of 6 steps with dt re-set every step); mean/std/count of c over
+    wrapping boxes of fluid cells agree to 1e-12 (fixed-order tree sums against index-order sums)."""
+    case = cases.duct_room(64, 32, 32)
+    s = binding.solver_for_case(case)
+    o = oracle_for(case)
+    assert s.courant() == o.courant() > 0
+    for _ in range(6):
+        s.step(1)
+        o.step(1)
+        co_s, co_o = s.courant(), o.courant()
+        assert abs(co_s - co_o) <= 1e-11 * co_o
+        dt = 0.4 * o.P.dt / co_o            # AdjustDt: hold the Courant number at 0.4 (decided on the oracle's value)
+        s.set_dt(dt)
+        o.set_dt(dt)
+    compare(s.fields_numpy(), o.fields(), TOL100, mask=case["mask"], what="courant-limited run")
+    nz, ny, nx = case["shape"]
+    for lo, size in [((0, 0, 0), (nx, ny, nz)), ((60, 30, 28), (9, 7, 11)), ((5, 6, 7), (1, 1, 1)), ((0, 0, 0), (2, ny, nz))]:
+        ms, ss, ns = s.scalar_stats(lo, size)
+        mo, so, no = o.scalar_stats(lo, size)
+        assert ns == no and abs(ms - mo) <= 1e-12 * max(abs(mo), 1e-300) + 1e-15 and abs(ss - so) <= 1e-12 * max(so, 1.0), (lo, size)
+    with pytest.raises(binding.DnslabError):
+        s.set_dt(0.0)
+    with pytest.raises(binding.DnslabError):
+        s.scalar_stats((0, 0, 0), (nx + 1, 1, 1))
+    s.close()
+    # unmasked, large: bit-identical maximum again, full-box statistics
+    case = cases.periodic_turbulence(64, steps=1)
+    s = binding.solver_for_case(case)
+    o = oracle_for(case)
+    assert s.courant() == o.courant()
+    ms, ss, ns = s.scalar_stats((0, 0, 0), (64, 64, 64))
+    mo, so, no = o.scalar_stats((0, 0, 0), (64, 64, 64))
+    assert ns == no == 64 ** 3 and abs(ms - mo) <= 1e-14 and abs(ss - so) <= 1e-12 * so
+    s.close()
+
+
 def test_two_stage_rk_kernel_variant():
     """flags bit 3: stages 1+2 and 3+4 fused (k_rk_pair, intermediate stage field in shared memory) -- same method,
     same tolerances; masked with sources, unmasked, a grid of one tile in x, and a z extent of one chunk."""
