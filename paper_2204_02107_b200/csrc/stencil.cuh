@@ -270,18 +270,27 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
         for (int m = 0; m < 4; ++m) zm[m] = __ldg(reinterpret_cast<const double2 *>(a.qs[m] + pkm + orow));
     }
     const int own = (ty + 1) * SW + 2 + 2 * tx; // this thread's pair inside a field's tile
+    unsigned fraw_next = 0x7f7f;
+    if (MASKED) fraw_next = *reinterpret_cast<const unsigned short *>(a.face + plane * (size_t)k0 + orow);
+    // sources whose x and y factors are non-zero at this thread's cells (their z factor is checked per plane)
+    unsigned smask = 0;
+    if (SOURCES) {
+        for (int s = 0; s < a.nsrc; ++s) {
+            const double *tb = a.stab + a.src[s].off;
+            const double2 sx = __ldg(reinterpret_cast<const double2 *>(tb + i));
+            if ((sx.x != 0.0 || sx.y != 0.0) && __ldg(&tb[nx + j]) != 0.0) smask |= 1u << s;
+        }
+    }
 
     for (int t = 0; t < kc; ++t) {
         const int k = k0 + t;
         const size_t o = plane * (size_t)k + orow;
         // operands that do not go through shared memory: issue their loads before waiting
         double2 qn[4], q2[4], q3[4];
-        unsigned fA = 0x7f, fB = 0x7f;
-        if (MASKED) {
-            const uchar2 fv = *reinterpret_cast<const uchar2 *>(a.face + o);
-            fA = fv.x;
-            fB = fv.y;
-        }
+        // face bytes: fetched one plane ahead and left packed until here, so the load is never waited for
+        const unsigned fraw = fraw_next;
+        if (MASKED && t + 1 < kc) fraw_next = *reinterpret_cast<const unsigned short *>(a.face + o + plane);
+        const unsigned fA = fraw & 0xffu, fB = fraw >> 8;
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
             if (STAGE >= 2) qn[m] = __ldg(reinterpret_cast<const double2 *>(a.qn[m] + o));
@@ -381,10 +390,11 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
             F[m] = make_double2(vx, vy);
         }
         if (SOURCES) {
-            for (int s = 0; s < a.nsrc; ++s) {
+            for (unsigned sm_ = smask; sm_; sm_ &= sm_ - 1) {
+                const int s = __ffs(sm_) - 1;
                 const double *tb = a.stab + a.src[s].off;
                 const double sz = __ldg(&tb[nx + ny + k]), sy = __ldg(&tb[nx + j]);
-                if (sy == 0.0 || sz == 0.0) continue;
+                if (sz == 0.0) continue;
                 const double2 sx = __ldg(reinterpret_cast<const double2 *>(tb + i));
                 const double SA = sx.x * sy * sz, SB = sx.y * sy * sz;
                 const uint32_t comps = a.src[s].comps;
