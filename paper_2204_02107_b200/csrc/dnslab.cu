@@ -380,7 +380,7 @@ template <int DIR> int launch_fft_col(dnslab *h, c2 *data, int axis)
 
 template <int L, int XT> int launch_fft_z_solve_LX(dnslab *h, c2 *data)
 {
-    constexpr int T = L / dnsfft::ElemsPerThread<L>::value;
+    constexpr int T = L / dnsfft::ElemsPerThreadZ<L>::value;
     constexpr int NT = XT * T < 32 ? 32 : XT * T;
     const int mx = h->P.nx / 2;
     const size_t smem = 2 * (size_t)XT * L * sizeof(c2);

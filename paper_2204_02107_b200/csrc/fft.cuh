@@ -72,6 +72,44 @@ template <int DIR> __device__ __forceinline__ void dft8(c2 (&v)[8])
     v[7] = csub(e3, o3);
 }
 
+// 16-point transform as 4 x 4: y[b][c] = sum_a v[4a+b] w4^(ac), times w16^(bc), then X[c+4d] = sum_b y[b][c] w4^(bd).
+template <int DIR> __device__ __forceinline__ c2 mul_w16(c2 a, int p) // a * w16^p, w16 = exp(-+2 pi i/16), p compile-time after unrolling
+{
+    const double c1 = 0.92387953251128675613, s1 = 0.38268343236508977173, h = 0.70710678118654752440;
+    double wr, wi; // forward twiddle (cos, -sin)
+    switch (p) {
+    case 0: return a;
+    case 1: wr = c1; wi = -s1; break;
+    case 2: wr = h; wi = -h; break;
+    case 3: wr = s1; wi = -c1; break;
+    case 4: return rot90<DIR>(a);
+    case 6: wr = -h; wi = -h; break;
+    default: wr = -c1; wi = s1; break; // 9
+    }
+    return DIR < 0 ? make_double2(a.x * wr - a.y * wi, a.x * wi + a.y * wr) : make_double2(a.x * wr + a.y * wi, a.y * wr - a.x * wi);
+}
+
+template <int DIR> __device__ __forceinline__ void dft16(c2 (&v)[16])
+{
+#pragma unroll
+    for (int b = 0; b < 4; ++b) dft4<DIR>(v[b], v[4 + b], v[8 + b], v[12 + b]); // v[4c+b] = y[b][c]
+#pragma unroll
+    for (int b = 1; b < 4; ++b)
+#pragma unroll
+        for (int c = 1; c < 4; ++c) v[4 * c + b] = mul_w16<DIR>(v[4 * c + b], b * c);
+#pragma unroll
+    for (int c = 0; c < 4; ++c) dft4<DIR>(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]); // v[4c+d] = X[c+4d]
+    // transpose the 4 x 4 index so that v[k] = X[k]
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int d = c + 1; d < 4; ++d) {
+            const c2 t = v[4 * c + d];
+            v[4 * c + d] = v[4 * d + c];
+            v[4 * d + c] = t;
+        }
+}
+
 // One Stockham stage of radix R on the E register elements of thread `tid` (element e <-> index
 // tid + e*T).  Ns = product of the radices of the earlier stages.  On exit slot q + r*(E/R) holds
 // output r of butterfly jj = tid + q*T, whose natural position is oidx = expand(jj) + r*Ns.
@@ -94,11 +132,16 @@ template <int L, int E, int R, int NS, int DIR, bool TWPOW> __device__ __forcein
                 w[1] = __ldg(&tw[kb]);
                 w[2] = cmul(w[1], w[1]);
                 w[3] = cmul(w[2], w[1]);
-                if constexpr (R == 8) {
+                if constexpr (R >= 8) {
                     w[4] = cmul(w[2], w[2]);
                     w[5] = cmul(w[4], w[1]);
                     w[6] = cmul(w[4], w[2]);
                     w[7] = cmul(w[4], w[3]);
+                }
+                if constexpr (R == 16) {
+                    w[8] = cmul(w[4], w[4]);
+#pragma unroll
+                    for (int r = 9; r < 16; ++r) w[r] = cmul(w[8], w[r - 8]);
                 }
 #pragma unroll
                 for (int r = 1; r < R; ++r) v[r] = twmul<DIR>(v[r], w[r]);
@@ -107,7 +150,9 @@ template <int L, int E, int R, int NS, int DIR, bool TWPOW> __device__ __forcein
                 for (int r = 1; r < R; ++r) v[r] = twmul<DIR>(v[r], __ldg(&tw[kb * r]));
             }
         }
-        if constexpr (R == 8) {
+        if constexpr (R == 16) {
+            dft16<DIR>(v);
+        } else if constexpr (R == 8) {
             dft8<DIR>(v);
         } else if constexpr (R == 4) {
             dft4<DIR>(v[0], v[1], v[2], v[3]);
@@ -121,7 +166,8 @@ template <int L, int E, int R, int NS, int DIR, bool TWPOW> __device__ __forcein
 
 template <int L, int E, int NS> struct NextRadix {
     static constexpr int rem = L / NS;
-    static constexpr int value = rem >= 8 ? (E >= 8 ? 8 : E) : rem;
+    static constexpr int cap = E >= 16 ? 16 : (E >= 8 ? 8 : E);
+    static constexpr int value = rem >= cap ? cap : rem;
 };
 
 // Full transform of one line held as x[e] <-> element tid + e*T, exchanging through `sm`
@@ -174,6 +220,8 @@ template <int XT> struct SmCol {
 };
 
 template <int L> struct ElemsPerThread { static constexpr int value = L >= 8 ? 8 : L; };
+// the fused z pass holds 16 elements per thread: one exchange per transform for L <= 256 (radix 16 x 16)
+template <int L> struct ElemsPerThreadZ { static constexpr int value = L >= 16 ? 16 : L; };
 
 // ---------------------------------------------------------------------------------------
 // Right-hand side of eq. 9 at one cell: r = d + sum_a delta_a[(1-beta) delta_a p].
@@ -284,11 +332,11 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThread<L>::value) < 32 ? 32 :
 // null modes (m = 0, 2ky = 0 mod ny, 2kz = 0 mod nz) set to 0, scaling by 1/N, inverse transform.
 // The tile index enumerates (x tile, ky).
 template <int L, int XT>
-__global__ void __launch_bounds__(XT *(L / ElemsPerThread<L>::value) < 32 ? 32 : XT *(L / ElemsPerThread<L>::value))
+__global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 : XT *(L / ElemsPerThreadZ<L>::value))
     k_fft_z_solve(c2 *__restrict__ data, const c2 *__restrict__ tw, int mx, int ny, const double *__restrict__ ex,
                   const double *__restrict__ ey, const double *__restrict__ ez, double inv_n, int ntiles)
 {
-    constexpr int E = ElemsPerThread<L>::value;
+    constexpr int E = ElemsPerThreadZ<L>::value;
     constexpr int T = L / E;
     extern __shared__ double2 smem[];
     const int tx = threadIdx.x % XT;
