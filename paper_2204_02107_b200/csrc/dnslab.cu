@@ -343,7 +343,7 @@ template <int DIR, bool PRO> int launch_fft_x(dnslab *h, const c2 *in, c2 *out, 
 // y pass: axis 1; z pass (unfused, used only by tests of the transform itself): axis 2
 template <int L, int XT, int DIR> int launch_fft_col_LX(dnslab *h, c2 *data, int axis)
 {
-    constexpr int T = L / dnsfft::ElemsPerThread<L>::value;
+    constexpr int T = L / dnsfft::ElemsPerThreadZ<L>::value;
     const int mx = h->P.nx / 2;
     const size_t stride = axis == 1 ? (size_t)mx : (size_t)mx * h->P.ny;
     const size_t other_stride = axis == 1 ? (size_t)mx * h->P.ny : (size_t)mx;

@@ -306,10 +306,10 @@ __global__ void __launch_bounds__(256) k_fft_x(const c2 *__restrict__ in, c2 *__
 // y or z pass, in place: XT adjacent x (complex) by L elements along the axis; element n of
 // column tx is at base + n*stride + tx.  blockIdx.x enumerates (x tile, other index).
 template <int L, int XT, int DIR>
-__global__ void __launch_bounds__(XT *(L / ElemsPerThread<L>::value) < 32 ? 32 : XT *(L / ElemsPerThread<L>::value))
+__global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 : XT *(L / ElemsPerThreadZ<L>::value))
     k_fft_col(c2 *__restrict__ data, const c2 *__restrict__ tw, int mx, size_t stride, size_t other_stride)
 {
-    constexpr int E = ElemsPerThread<L>::value;
+    constexpr int E = ElemsPerThreadZ<L>::value;
     constexpr int T = L / E;
     extern __shared__ double2 smem[];
     const int tx = threadIdx.x % XT;
