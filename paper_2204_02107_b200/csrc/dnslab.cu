@@ -313,10 +313,10 @@ template <typename K> int persistent_grid(dnslab *h, K kernel, int threads, size
 
 template <int L, int DIR, bool PRO> int launch_fft_x_L(dnslab *h, const c2 *in, c2 *out, const dnsfft::PoissonRhsArgs &ra)
 {
-    constexpr int E = dnsfft::ElemsPerThread<L>::value;
+    constexpr int E = dnsfft::ElemsPerThreadZ<L>::value;
     constexpr int T = L / E;
     const size_t nlines = (size_t)h->P.ny * h->P.nz;
-    size_t nl = 256 / T;
+    size_t nl = 128 / T;
     if (nl > nlines) nl = nlines;
     const size_t smem = nl * (L + L / 8) * sizeof(c2);
     ProfScope ps(h, DNSLAB_K_FFT_X);

@@ -273,7 +273,7 @@ template <int L, int DIR, bool PROLOGUE>
 __global__ void __launch_bounds__(256) k_fft_x(const c2 *__restrict__ in, c2 *__restrict__ out, const c2 *__restrict__ tw, int nlines_per_block,
                                                PoissonRhsArgs ra)
 {
-    constexpr int E = ElemsPerThread<L>::value;
+    constexpr int E = ElemsPerThreadZ<L>::value;
     constexpr int T = L / E;
     extern __shared__ double2 smem[];
     const int lt = threadIdx.x / T; // line within block
