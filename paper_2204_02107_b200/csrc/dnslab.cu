@@ -438,9 +438,15 @@ int poisson_solve(dnslab *h, const double *d, const double *pold, double *pout, 
 
 int launch_div(dnslab *h, double *const *q)
 {
+    ProfScope ps(h, DNSLAB_K_DIV);
+    if (h->P.nx >= 64 && h->P.ny >= 8) {
+        const dim3 blk2(32, 8, 1), grd2(h->P.nx / 64, h->P.ny / 8, h->P.nz);
+        dnsst::k_div2<<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], h->d, h->P.nx, h->P.ny, h->P.nz, 1.0 / (2.0 * h->P.dx),
+                                                    1.0 / (2.0 * h->P.dy), 1.0 / (2.0 * h->P.dz));
+        return check_launch(h);
+    }
     const dim3 blk = tile_block(h);
     const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz);
-    ProfScope ps(h, DNSLAB_K_DIV);
     dnsst::k_div<<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], h->d, h->P.nx, h->P.ny, h->P.nz, 1.0 / (2.0 * h->P.dx),
                                               1.0 / (2.0 * h->P.dy), 1.0 / (2.0 * h->P.dz));
     return check_launch(h);
@@ -452,6 +458,12 @@ int launch_project(dnslab *h, double *const *q, const double *p)
     const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz);
     const double r2x = 1.0 / (2.0 * h->P.dx), r2y = 1.0 / (2.0 * h->P.dy), r2z = 1.0 / (2.0 * h->P.dz);
     ProfScope ps(h, DNSLAB_K_PROJECT);
+    if (h->P.nx >= 64 && h->P.ny >= 8) {
+        const dim3 blk2(32, 8, 1), grd2(h->P.nx / 64, h->P.ny / 8, h->P.nz);
+        if (h->face) dnsst::k_project2<true><<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], p, h->face, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
+        else dnsst::k_project2<false><<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], p, nullptr, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
+        return check_launch(h);
+    }
     if (h->face) dnsst::k_project<true><<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], p, h->face, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
     else dnsst::k_project<false><<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], p, nullptr, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
     return check_launch(h);

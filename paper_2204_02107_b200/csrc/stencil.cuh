@@ -1013,6 +1013,54 @@ template <bool MASKED> __global__ void __launch_bounds__(256) k_filter_march(con
     }
 }
 
+// a4 and a6 with two x-adjacent cells per thread (16-byte accesses, twice the bytes in flight per thread); nx >= 64.
+// blockDim = (32, 8): a block covers 64 x 8 cells of one plane.
+__global__ void __launch_bounds__(256) k_div2(const double *__restrict__ u, const double *__restrict__ v, const double *__restrict__ w,
+                                              double *__restrict__ d, int nx, int ny, int nz, double r2x, double r2y, double r2z)
+{
+    const int i = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+    const int j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    const size_t plane = (size_t)nx * ny, pk = plane * k, row = pk + (size_t)nx * j;
+    const double2 vp = __ldg(reinterpret_cast<const double2 *>(v + pk + (size_t)nx * ((j + 1) & (ny - 1)) + i));
+    const double2 vm = __ldg(reinterpret_cast<const double2 *>(v + pk + (size_t)nx * ((j - 1) & (ny - 1)) + i));
+    const double2 wp = __ldg(reinterpret_cast<const double2 *>(w + plane * ((k + 1) & (nz - 1)) + (size_t)nx * j + i));
+    const double2 wm = __ldg(reinterpret_cast<const double2 *>(w + plane * ((k - 1) & (nz - 1)) + (size_t)nx * j + i));
+    const double2 uc = __ldg(reinterpret_cast<const double2 *>(u + row + i));
+    const double um = __ldg(u + row + ((i - 1) & (nx - 1))), up = __ldg(u + row + ((i + 2) & (nx - 1)));
+    double2 r;
+    r.x = (uc.y - um) * r2x + (vp.x - vm.x) * r2y + (wp.x - wm.x) * r2z;
+    r.y = (up - uc.x) * r2x + (vp.y - vm.y) * r2y + (wp.y - wm.y) * r2z;
+    *reinterpret_cast<double2 *>(d + row + i) = r;
+}
+
+template <bool MASKED>
+__global__ void __launch_bounds__(256) k_project2(double *__restrict__ u, double *__restrict__ v, double *__restrict__ w, const double *__restrict__ p,
+                                                  const uint8_t *__restrict__ face, int nx, int ny, int nz, double r2x, double r2y, double r2z)
+{
+    const int i = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+    const int j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    const size_t plane = (size_t)nx * ny, pk = plane * k, row = pk + (size_t)nx * j, o = row + i;
+    unsigned f = 0x0101;
+    if (MASKED) f = *reinterpret_cast<const unsigned short *>(face + o);
+    const double2 pyp = __ldg(reinterpret_cast<const double2 *>(p + pk + (size_t)nx * ((j + 1) & (ny - 1)) + i));
+    const double2 pym = __ldg(reinterpret_cast<const double2 *>(p + pk + (size_t)nx * ((j - 1) & (ny - 1)) + i));
+    const double2 pzp = __ldg(reinterpret_cast<const double2 *>(p + plane * ((k + 1) & (nz - 1)) + (size_t)nx * j + i));
+    const double2 pzm = __ldg(reinterpret_cast<const double2 *>(p + plane * ((k - 1) & (nz - 1)) + (size_t)nx * j + i));
+    const double2 pc = __ldg(reinterpret_cast<const double2 *>(p + o));
+    const double pm = __ldg(p + row + ((i - 1) & (nx - 1))), pp = __ldg(p + row + ((i + 2) & (nx - 1)));
+    double2 uu = *reinterpret_cast<const double2 *>(u + o), vv = *reinterpret_cast<const double2 *>(v + o), ww = *reinterpret_cast<const double2 *>(w + o);
+    const bool fa = (f & 1) != 0, fb = (f & 0x100) != 0;
+    uu.x = fa ? uu.x - (pc.y - pm) * r2x : 0.0;
+    uu.y = fb ? uu.y - (pp - pc.x) * r2x : 0.0;
+    vv.x = fa ? vv.x - (pyp.x - pym.x) * r2y : 0.0;
+    vv.y = fb ? vv.y - (pyp.y - pym.y) * r2y : 0.0;
+    ww.x = fa ? ww.x - (pzp.x - pzm.x) * r2z : 0.0;
+    ww.y = fb ? ww.y - (pzp.y - pzm.y) * r2z : 0.0;
+    *reinterpret_cast<double2 *>(u + o) = uu;
+    *reinterpret_cast<double2 *>(v + o) = vv;
+    *reinterpret_cast<double2 *>(w + o) = ww;
+}
+
 // a6: u_a = beta ? u*_a - delta_a p : +0.0, in place (eq. 8)
 template <bool MASKED>
 __global__ void __launch_bounds__(256) k_project(double *__restrict__ u, double *__restrict__ v, double *__restrict__ w, const double *__restrict__ p,
