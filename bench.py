@@ -36,7 +36,7 @@ def canonical_bytes_per_cell(P, masked):
 # Bytes per cell per launch of each kernel class.
 # "canonical": SURVEY.md 8(d)'s model (accumulate-form RK with Qc: 12+20+20+12 passes; div R3 W1; 5 FFT passes of
 # R1 W1 per solve; dense p^k + mask read per eq. 9 iteration; projection R4 W3).
-# "moved": what this implementation must move (Qc eliminated: 8+12+12+20 passes; eq. 9 only at the near-solid
+# "moved": what this implementation must move (Qc eliminated: 8+16+12+12 passes; eq. 9 only at the near-solid
 # cells, a fraction fb of the grid: index 4 + saved d 8 + d 8 + p centre 8 + face 1 + ~1 neighbour 8 bytes).
 def class_bytes_per_cell(masked, fb=0.0):
     m = 0.125 if masked else 0.0
@@ -51,7 +51,7 @@ def class_bytes_per_cell(masked, fb=0.0):
         "filter": 64.0 + m,
     }
     moved = dict(canonical)
-    moved["rk_stage"] = (64 + 96 + 96 + 160) / 4.0 + (1.0 if masked else 0.0)
+    moved["rk_stage"] = (64 + 128 + 96 + 96) / 4.0 + (1.0 if masked else 0.0)   # stage 2 also writes S; stage 4 reads Q4, S
     moved["project"] = 56.0 + (1.0 if masked else 0.0)
     moved["eq9_sparse"] = 37.0 * fb
     moved["filter"] = 64.0 + (1.0 if masked else 0.0)

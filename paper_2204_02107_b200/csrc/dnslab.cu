@@ -758,19 +758,19 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
             if ((rc = launch_rk_pair<0>(h, h->Q, h->A, h->Bf))) return rc;
             if ((rc = launch_rk_pair<1>(h, h->Bf, h->A, h->Bf))) return rc;
         } else if (!stage_proj) {
-            // Qc eliminated: A = Q2 (then Q*), Bf = Q3, Qc = Q4
+            // Qc eliminated: A = Q2, Bf = Q3, Qc = S = Q2 - Qn + 2 Q3 (written by stage 2), A = Q4, Q* in place of S
             if ((rc = launch_rk<1, true>(h, h->Q, h->A, nullptr, nullptr))) return rc;
-            if ((rc = launch_rk<2, true>(h, h->A, h->Bf, nullptr, nullptr))) return rc;
-            if ((rc = launch_rk<3, true>(h, h->Bf, h->Qc, nullptr, nullptr))) return rc;
-            if ((rc = launch_rk<4, true>(h, h->Qc, nullptr, h->A, h->Bf))) return rc;
+            if ((rc = launch_rk<2, true>(h, h->A, h->Bf, h->Qc, nullptr))) return rc;
+            if ((rc = launch_rk<3, true>(h, h->Bf, h->A, nullptr, nullptr))) return rc;
+            if ((rc = launch_rk<4, true>(h, h->A, nullptr, h->Qc, nullptr))) return rc;
         }
         if (!stage_proj) {
-            if ((rc = pressure_stage(h, h->A, h->p))) return rc;
-            // new state: A, or (flags bit 0) its filtered copy in Qc, which this path does not use otherwise
-            double **fin = h->A;
+            // Q* is in A (two-stage kernels) or Qc (one kernel per stage); the other one is free for the filter
+            double **fin = h->pair_kc > 0 ? h->A : h->Qc, **spare = h->pair_kc > 0 ? h->Qc : h->A;
+            if ((rc = pressure_stage(h, fin, h->p))) return rc;
             if (filter) {
-                if ((rc = launch_filter(h, h->A, h->Qc))) return rc;
-                fin = h->Qc;
+                if ((rc = launch_filter(h, fin, spare))) return rc;
+                fin = spare;
             }
             for (int m = 0; m < 4; ++m) {
                 double *t = h->Q[m];

@@ -55,10 +55,10 @@ struct PairCoef {
 struct RKArgs {
     const double *qs[4]; // stage field (stencil input)
     const double *qn[4]; // Q^n
-    const double *qc[4]; // running combination Qc, read (stages 2-4); with ELIM at stage 4: Q2
-    const double *q3[4]; // ELIM, stage 4 only: Q3
+    const double *qc[4]; // running combination Qc, read (stages 2-4); with ELIM at stage 4: S = Q2 - Qn + 2 Q3
+    const double *q3[4]; // unused
     double *qo[4];       // next stage field, written (stages 1-3)
-    double *qco[4];      // Qc written (accumulate form); with ELIM at stage 4: Q* (aliases Q2)
+    double *qco[4];      // Qc written (accumulate form); with ELIM: S at stage 2, Q* at stage 4 (in place of S)
     const uint8_t *face; // null: no solid cells
     int nx, ny, nz;
     double r2x, r2y, r2z;    // 1/(2 D_a)
@@ -78,11 +78,11 @@ struct RKArgs {
 // through L1 (DRAM traffic stays at the compulsory bytes, see profiles/).
 //
 // ELIM = false, the accumulate form of the oracle:   Qc (+)= b_s dt F ;  Qs' = Qn + a_s dt F.
-// ELIM = true, Qc eliminated algebraically (12 fewer field passes per step):
-//     stages 1-3:  Qs' = Qn + a_s dt F
-//     stage 4:     Q*  = (-Qn + Q2 + 2 Q3 + Q4)/3 + (dt/6) F4
+// ELIM = true, Qc eliminated algebraically (48 instead of 65 field passes per step):
+//     stages 1-3:  Qs' = Qn + a_s dt F;   stage 2 also writes  S = Q2 - Qn + 2 Q3  (it holds all three)
+//     stage 4:     Q*  = (S + Q4)/3 + (dt/6) F4,  in place of S
 //   which equals Qn + dt/6 (F1 + 2 F2 + 2 F3 + F4) because Q2 = Qn + dt/2 F1, Q3 = Qn + dt/2 F2,
-//   Q4 = Qn + dt F3 (classical RK4).  Q* overwrites Q2 in place.
+//   Q4 = Qn + dt F3 (classical RK4).  Stage 4 then reads two fields sets, not four.
 template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __launch_bounds__(256, 3) k_rk(const RKArgs a)
 {
     const int nx = a.nx, ny = a.ny, nz = a.nz;
@@ -97,7 +97,7 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
     const size_t ozp = plane * ((k + 1) & (nz - 1)) + rowc + i, ozm = plane * ((k - 1) & (nz - 1)) + rowc + i;
     unsigned f = 0x7f;
     if (MASKED) f = a.face[o];
-    double f0[4], xp[4], xm[4], yp[4], ym[4], fp[4], fm[4], qn[4], qc[4], q3[4];
+    double f0[4], xp[4], xm[4], yp[4], ym[4], fp[4], fm[4], qn[4], qc[4];
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
         f0[m] = __ldg(&a.qs[m][o]);
@@ -108,13 +108,10 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
         fp[m] = __ldg(&a.qs[m][ozp]);
         fm[m] = __ldg(&a.qs[m][ozm]);
         qn[m] = f0[m];
-        if (STAGE >= 2 && (STAGE <= 3 || ELIM)) qn[m] = __ldg(&a.qn[m][o]);
+        if (STAGE >= 2 && (STAGE <= 3 || !ELIM)) qn[m] = __ldg(&a.qn[m][o]);
         qc[m] = qn[m];
         if (STAGE >= 2 && !ELIM) qc[m] = a.qc[m][o]; // plain loads: updated in place
-        if (STAGE == 4 && ELIM) {
-            qc[m] = a.qc[m][o]; // Q2, overwritten below by Q*
-            q3[m] = __ldg(&a.q3[m][o]);
-        }
+        if (STAGE == 4 && ELIM) qc[m] = a.qc[m][o]; // S, overwritten below by Q*
     }
     double F[4];
     if (!MASKED || (f & 1)) {
@@ -157,8 +154,13 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
             if (ELIM) {
-                if (STAGE < 4) a.qo[m][o] = qn[m] + a.ca * F[m];
-                else a.qco[m][o] = (qc[m] - qn[m] + 2.0 * q3[m] + f0[m]) * (1.0 / 3.0) + a.cb * F[m];
+                if (STAGE < 4) {
+                    const double r = qn[m] + a.ca * F[m];
+                    a.qo[m][o] = r;
+                    if (STAGE == 2) a.qco[m][o] = (f0[m] - qn[m]) + 2.0 * r;
+                } else {
+                    a.qco[m][o] = (qc[m] + f0[m]) * (1.0 / 3.0) + a.cb * F[m];
+                }
             } else {
                 a.qco[m][o] = qc[m] + a.cb * F[m];
                 if (STAGE < 4) a.qo[m][o] = qn[m] + a.ca * F[m];
@@ -168,7 +170,7 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
         // solid cell: every field it holds is +0.0 and stays +0.0 (select)
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            if (!ELIM || STAGE == 4) a.qco[m][o] = 0.0;
+            if (!ELIM || STAGE == 4 || STAGE == 2) a.qco[m][o] = 0.0;
             if (STAGE < 4) a.qo[m][o] = 0.0;
         }
     }
@@ -286,19 +288,16 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
         const int k = k0 + t;
         const size_t o = plane * (size_t)k + orow;
         // operands that do not go through shared memory: issue their loads before waiting
-        double2 qn[4], q2[4], q3[4];
+        double2 qn[4], q2[4];
         // face bytes: fetched one plane ahead and left packed until here, so the load is never waited for
         const unsigned fraw = fraw_next;
         if (MASKED && t + 1 < kc) fraw_next = *reinterpret_cast<const unsigned short *>(a.face + o + plane);
         const unsigned fA = fraw & 0xffu, fB = fraw >> 8;
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            if (STAGE >= 2) qn[m] = __ldg(reinterpret_cast<const double2 *>(a.qn[m] + o));
+            if (STAGE >= 2 && (STAGE <= 3 || !ELIM)) qn[m] = __ldg(reinterpret_cast<const double2 *>(a.qn[m] + o));
             if (STAGE >= 2 && !ELIM) q2[m] = *reinterpret_cast<const double2 *>(a.qc[m] + o); // Qc, updated in place
-            if (STAGE == 4 && ELIM) {
-                q2[m] = *reinterpret_cast<const double2 *>(a.qc[m] + o); // Q2, overwritten below by Q*
-                q3[m] = __ldg(reinterpret_cast<const double2 *>(a.q3[m] + o));
-            }
+            if (STAGE == 4 && ELIM) q2[m] = *reinterpret_cast<const double2 *>(a.qc[m] + o);  // S, overwritten below by Q*
         }
         cp_async_wait_one();
         __syncthreads(); // plane k+1 visible to all; every thread is done with the tile of plane k-1
@@ -416,9 +415,15 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
                     r.x = flA ? qn[m].x + a.ca * F[m].x : 0.0;
                     r.y = flB ? qn[m].y + a.ca * F[m].y : 0.0;
                     *reinterpret_cast<double2 *>(a.qo[m] + o) = r;
+                    if (STAGE == 2) { // S = Q2 - Qn + 2 Q3 (all +0.0 in solid cells)
+                        double2 sv;
+                        sv.x = flA ? (cur[m].x - qn[m].x) + 2.0 * r.x : 0.0;
+                        sv.y = flB ? (cur[m].y - qn[m].y) + 2.0 * r.y : 0.0;
+                        *reinterpret_cast<double2 *>(a.qco[m] + o) = sv;
+                    }
                 } else {
-                    r.x = flA ? (q2[m].x - qn[m].x + 2.0 * q3[m].x + cur[m].x) * (1.0 / 3.0) + a.cb * F[m].x : 0.0;
-                    r.y = flB ? (q2[m].y - qn[m].y + 2.0 * q3[m].y + cur[m].y) * (1.0 / 3.0) + a.cb * F[m].y : 0.0;
+                    r.x = flA ? (q2[m].x + cur[m].x) * (1.0 / 3.0) + a.cb * F[m].x : 0.0;
+                    r.y = flB ? (q2[m].y + cur[m].y) * (1.0 / 3.0) + a.cb * F[m].y : 0.0;
                     *reinterpret_cast<double2 *>(a.qco[m] + o) = r;
                 }
             } else {
