@@ -212,8 +212,9 @@ template <int T> struct SmLine {
     }
 };
 // column of a tile whose fastest index is the XT-wide x offset (y and z passes)
-template <int XT> struct SmCol {
-    static constexpr bool TWPOW = true;  // fewer look-ups pay here too (y pass of 512x256x128: 47.5 instead of 50.6 us)
+// TWP: twiddles of a butterfly as powers of one look-up (else one look-up each; lanes share them here)
+template <int XT, bool TWP = true> struct SmCol {
+    static constexpr bool TWPOW = TWP;
     c2 *base; // already offset by tx
     __device__ __forceinline__ c2 &at(int n) { return base[n * XT]; }
     __device__ __forceinline__ void sync() { __syncthreads(); }
