@@ -272,14 +272,15 @@ __device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_
 //   out-of-place or in-place (a line is read completely before it is written).
 template <int L, int DIR, bool PROLOGUE>
 __global__ void __launch_bounds__(256) k_fft_x(const c2 *__restrict__ in, c2 *__restrict__ out, const c2 *__restrict__ tw, int nlines_per_block,
-                                               PoissonRhsArgs ra)
+                                               int rev, PoissonRhsArgs ra)
 {
     constexpr int E = ElemsPerThreadZ<L>::value;
     constexpr int T = L / E;
     extern __shared__ double2 smem[];
     const int lt = threadIdx.x / T; // line within block
     const int tid = threadIdx.x - lt * T;
-    const size_t line = (size_t)blockIdx.x * nlines_per_block + lt;
+    // rev: walk the lines from the far end, so that a pass starts on what the pass before it left in L2
+    const size_t line = (size_t)(rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x) * nlines_per_block + lt;
     const c2 *src = in + line * L;
     c2 x[E];
 #pragma unroll
@@ -308,7 +309,7 @@ __global__ void __launch_bounds__(256) k_fft_x(const c2 *__restrict__ in, c2 *__
 // column tx is at base + n*stride + tx.  blockIdx.x enumerates (x tile, other index).
 template <int L, int XT, int DIR>
 __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 : XT *(L / ElemsPerThreadZ<L>::value))
-    k_fft_col(c2 *__restrict__ data, const c2 *__restrict__ tw, int mx, size_t stride, size_t other_stride)
+    k_fft_col(c2 *__restrict__ data, const c2 *__restrict__ tw, int mx, size_t stride, size_t other_stride, int rev)
 {
     constexpr int E = ElemsPerThreadZ<L>::value;
     constexpr int T = L / E;
@@ -316,8 +317,9 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 
     const int tx = threadIdx.x % XT;
     const int tid = threadIdx.x / XT;
     const int xtiles = mx / XT;
-    const int xt = blockIdx.x % xtiles;
-    const size_t other = blockIdx.x / xtiles;
+    const unsigned bid = rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const int xt = bid % xtiles;
+    const size_t other = bid / xtiles;
     c2 *base = data + other * other_stride + (size_t)xt * XT + tx;
     c2 x[E];
 #pragma unroll
@@ -335,7 +337,7 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 
 template <int L, int XT>
 __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 : XT *(L / ElemsPerThreadZ<L>::value))
     k_fft_z_solve(c2 *__restrict__ data, const c2 *__restrict__ tw, int mx, int ny, const double *__restrict__ ex,
-                  const double *__restrict__ ey, const double *__restrict__ ez, double inv_n, int ntiles)
+                  const double *__restrict__ ey, const double *__restrict__ ez, double inv_n, int ntiles, int rev)
 {
     constexpr int E = ElemsPerThreadZ<L>::value;
     constexpr int T = L / E;
@@ -344,7 +346,8 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 
     const int tid = threadIdx.x / XT;
     const int xtiles = mx / XT;
     const size_t stride = (size_t)mx * ny;
-    auto issue = [&](int tile, int b) {
+    auto issue = [&](int t_, int b) {
+        const int tile = rev ? ntiles - 1 - t_ : t_;
         const c2 *src = data + (size_t)(tile / xtiles) * mx + (tile % xtiles) * XT + tx;
         c2 *dst = smem + b * (XT * L) + tx;
 #pragma unroll
@@ -353,13 +356,14 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 
     double ezr[E]; // 1/N scaling folded in later; ez depends only on this thread's kz
 #pragma unroll
     for (int e = 0; e < E; ++e) ezr[e] = __ldg(&ez[tid + e * T]);
-    int tile = blockIdx.x, b = 0;
-    if (tile < ntiles) issue(tile, 0);
+    int lt_ = blockIdx.x, b = 0; // logical tile; the physical one counts from the far end when rev
+    if (lt_ < ntiles) issue(lt_, 0);
     cp_async_commit();
-    for (; tile < ntiles; tile += gridDim.x, b ^= 1) {
-        if (tile + (int)gridDim.x < ntiles) issue(tile + gridDim.x, b ^ 1);
+    for (; lt_ < ntiles; lt_ += gridDim.x, b ^= 1) {
+        if (lt_ + (int)gridDim.x < ntiles) issue(lt_ + gridDim.x, b ^ 1);
         cp_async_commit();
         cp_async_wait_1();
+        const int tile = rev ? ntiles - 1 - lt_ : lt_;
         const int ky = tile / xtiles, m = (tile % xtiles) * XT + tx;
         SmCol<XT> sm{smem + b * (XT * L) + tx};
         c2 x[E];
