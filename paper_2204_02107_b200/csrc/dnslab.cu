@@ -111,6 +111,7 @@ struct dnslab {
     int64_t launches;
     dim3 rk_block;
     int nsm;   // SM count of the device
+    int st_rev;  // bit per stencil kernel of a step (RK stages 1-4, divergence, projection): same idea
     int fft_rev; // bit per pass of a solve (x fwd, y fwd, z, y inv, x inv): walk its tiles from the far end
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
     int pair_kc; // > 0: two-stage kernel (k_rk_pair) with this many planes per block; 0: one launch per stage
@@ -219,6 +220,7 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
     if (h->rk_kc > 0) {
         // z-marching kernel: 64 x 8 columns, kc planes per block
         a.kc = h->rk_kc;
+        a.rev = (h->st_rev >> (STAGE - 1)) & 1;
         const dim3 blk(32, dnsst::RKM_TY, 1);
         const dim3 grd(h->P.nx / dnsst::RKM_TX, h->P.ny / dnsst::RKM_TY, h->P.nz / h->rk_kc);
         const size_t smem = dnsst::RKM_SMEM;
@@ -443,7 +445,7 @@ int launch_div(dnslab *h, double *const *q)
     if (h->P.nx >= 64 && h->P.ny >= 8) {
         const dim3 blk2(32, 8, 1), grd2(h->P.nx / 64, h->P.ny / 8, h->P.nz);
         dnsst::k_div2<<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], h->d, h->P.nx, h->P.ny, h->P.nz, 1.0 / (2.0 * h->P.dx),
-                                                    1.0 / (2.0 * h->P.dy), 1.0 / (2.0 * h->P.dz));
+                                                    1.0 / (2.0 * h->P.dy), 1.0 / (2.0 * h->P.dz), (h->st_rev >> 4) & 1);
         return check_launch(h);
     }
     const dim3 blk = tile_block(h);
@@ -461,8 +463,8 @@ int launch_project(dnslab *h, double *const *q, const double *p)
     ProfScope ps(h, DNSLAB_K_PROJECT);
     if (h->P.nx >= 64 && h->P.ny >= 8) {
         const dim3 blk2(32, 8, 1), grd2(h->P.nx / 64, h->P.ny / 8, h->P.nz);
-        if (h->face) dnsst::k_project2<true><<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], p, h->face, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
-        else dnsst::k_project2<false><<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], p, nullptr, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
+        if (h->face) dnsst::k_project2<true><<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], p, h->face, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z, (h->st_rev >> 5) & 1);
+        else dnsst::k_project2<false><<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], p, nullptr, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z, (h->st_rev >> 5) & 1);
         return check_launch(h);
     }
     if (h->face) dnsst::k_project<true><<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], p, h->face, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
@@ -580,6 +582,8 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
     h->nsm = prop.multiProcessorCount;
     h->fft_rev = 10; // y passes walk against the x passes: 41.7 instead of 45 us each (measured sweep over the 5-bit choices)
     if (const char *v = getenv("DNSLAB_FFT_REV")) h->fft_rev = atoi(v);
+    h->st_rev = 16; // only the divergence gains from it (83 instead of 88 us); the RK stages do not
+    if (const char *v = getenv("DNSLAB_ST_REV")) h->st_rev = atoi(v);
     h->ws = (char *)workspace;
     h->L = make_layout(params);
     const Layout &L = h->L;

@@ -68,6 +68,7 @@ struct RKArgs {
     double ca, cb;           // a_s dt, b_s dt
     int nsrc;
     int kc;                  // k_rk_march: planes per block
+    int rev;                 // k_rk_march: walk the y tiles and z chunks from the far end (start on what the kernel before left in L2)
     const double *stab;
     PairCoef kf;
     SourceDev src[DNS_MAX_SRC];
@@ -234,7 +235,8 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
     double *sm = reinterpret_cast<double *>(rkm_smem2);
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * 32 + tx;
     const int nx = a.nx, ny = a.ny, nz = a.nz, kc = a.kc;
-    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * RKM_TY, k0 = blockIdx.z * kc;
+    const int by = a.rev ? gridDim.y - 1 - blockIdx.y : blockIdx.y, bz = a.rev ? gridDim.z - 1 - blockIdx.z : blockIdx.z;
+    const int x0 = blockIdx.x * TX, y0 = by * RKM_TY, k0 = bz * kc;
     const int i = x0 + 2 * tx, j = y0 + ty;
     const size_t plane = (size_t)nx * ny;
     const size_t orow = (size_t)nx * j + i;
@@ -1021,10 +1023,10 @@ template <bool MASKED> __global__ void __launch_bounds__(256) k_filter_march(con
 // a4 and a6 with two x-adjacent cells per thread (16-byte accesses, twice the bytes in flight per thread); nx >= 64.
 // blockDim = (32, 8): a block covers 64 x 8 cells of one plane.
 __global__ void __launch_bounds__(256) k_div2(const double *__restrict__ u, const double *__restrict__ v, const double *__restrict__ w,
-                                              double *__restrict__ d, int nx, int ny, int nz, double r2x, double r2y, double r2z)
+                                              double *__restrict__ d, int nx, int ny, int nz, double r2x, double r2y, double r2z, int rev)
 {
     const int i = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
-    const int j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    const int j = (rev ? gridDim.y - 1 - blockIdx.y : blockIdx.y) * blockDim.y + threadIdx.y, k = rev ? gridDim.z - 1 - blockIdx.z : blockIdx.z;
     const size_t plane = (size_t)nx * ny, pk = plane * k, row = pk + (size_t)nx * j;
     const double2 vp = __ldg(reinterpret_cast<const double2 *>(v + pk + (size_t)nx * ((j + 1) & (ny - 1)) + i));
     const double2 vm = __ldg(reinterpret_cast<const double2 *>(v + pk + (size_t)nx * ((j - 1) & (ny - 1)) + i));
@@ -1040,10 +1042,10 @@ __global__ void __launch_bounds__(256) k_div2(const double *__restrict__ u, cons
 
 template <bool MASKED>
 __global__ void __launch_bounds__(256) k_project2(double *__restrict__ u, double *__restrict__ v, double *__restrict__ w, const double *__restrict__ p,
-                                                  const uint8_t *__restrict__ face, int nx, int ny, int nz, double r2x, double r2y, double r2z)
+                                                  const uint8_t *__restrict__ face, int nx, int ny, int nz, double r2x, double r2y, double r2z, int rev)
 {
     const int i = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
-    const int j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    const int j = (rev ? gridDim.y - 1 - blockIdx.y : blockIdx.y) * blockDim.y + threadIdx.y, k = rev ? gridDim.z - 1 - blockIdx.z : blockIdx.z;
     const size_t plane = (size_t)nx * ny, pk = plane * k, row = pk + (size_t)nx * j, o = row + i;
     unsigned f = 0x0101;
     if (MASKED) f = *reinterpret_cast<const unsigned short *>(face + o);
