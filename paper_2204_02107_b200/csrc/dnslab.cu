@@ -478,9 +478,11 @@ int launch_eq9_sparse(dnslab *h, const double *p, bool first)
     while ((1 << lgx) < h->P.nx) ++lgx;
     while ((1 << lgy) < h->P.ny) ++lgy;
     ProfScope ps(h, DNSLAB_K_EQ9);
-    dnsst::k_eq9_sparse<<<(unsigned)((h->nb + 255) / 256), 256, 0, h->stream>>>(h->d, p, h->face, h->blist, h->bsave, h->nb, first ? 1 : 0, h->P.nx,
-                                                                              h->P.ny, h->P.nz, lgx, lgy, 1.0 / (2.0 * h->P.dx),
-                                                                              1.0 / (2.0 * h->P.dy), 1.0 / (2.0 * h->P.dz));
+    const int per = 256 * dnsst::EQ9_ITEMS;
+    const unsigned grid = (unsigned)((h->nb + per - 1) / per);
+    const double r2x = 1.0 / (2.0 * h->P.dx), r2y = 1.0 / (2.0 * h->P.dy), r2z = 1.0 / (2.0 * h->P.dz);
+    if (first) dnsst::k_eq9_sparse<true><<<grid, 256, 0, h->stream>>>(h->d, p, h->face, h->blist, h->bsave, h->nb, h->P.nx, h->P.ny, h->P.nz, lgx, lgy, r2x, r2y, r2z);
+    else dnsst::k_eq9_sparse<false><<<grid, 256, 0, h->stream>>>(h->d, p, h->face, h->blist, h->bsave, h->nb, h->P.nx, h->P.ny, h->P.nz, lgx, lgy, r2x, r2y, r2z);
     return check_launch(h);
 }
 

@@ -855,32 +855,50 @@ __global__ void __launch_bounds__(256) k_div(const double *__restrict__ u, const
 // The first iteration of a step saves d at those cells (`save`), later ones restore it from there, and
 // r overwrites d in place: everywhere else r == d already, so the forward x pass reads one plain array.
 // face: bit0 beta(cell), bit1/2 beta(x+1/x-1), bit3/4 beta(y+1/y-1), bit5/6 beta(z+1/z-1).
+constexpr int EQ9_ITEMS = 4; // list entries per thread: their loads are issued together (the kernel is a latency-bound gather)
+template <bool FIRST>
 __global__ void __launch_bounds__(256) k_eq9_sparse(double *__restrict__ d, const double *__restrict__ p, const uint8_t *__restrict__ face,
-                                                    const uint32_t *__restrict__ list, double *__restrict__ save, int nlist, int first,
-                                                    int nx, int ny, int nz, int lgx, int lgy, double r2x, double r2y, double r2z)
+                                                    const uint32_t *__restrict__ list, double *__restrict__ save, int nlist, int nx, int ny,
+                                                    int nz, int lgx, int lgy, double r2x, double r2y, double r2z)
 {
-    const int n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= nlist) return;
-    const uint32_t o = list[n];
-    const int i = o & (nx - 1), j = (o >> lgx) & (ny - 1), k = o >> (lgx + lgy);
-    const unsigned f = face[o];
-    double dv;
-    if (first) {
-        dv = d[o];
-        save[n] = dv;
-    } else {
-        dv = save[n];
+    const int base = blockIdx.x * (256 * EQ9_ITEMS) + threadIdx.x;
+    uint32_t o[EQ9_ITEMS];
+    unsigned f[EQ9_ITEMS];
+    double dv[EQ9_ITEMS], pc[EQ9_ITEMS];
+#pragma unroll
+    for (int it = 0; it < EQ9_ITEMS; ++it) {
+        const int n = base + it * 256;
+        o[it] = n < nlist ? __ldg(&list[n]) : 0u;
     }
-    const size_t row = (size_t)nx * ((size_t)j + (size_t)ny * k);
-    const double pc = __ldg(&p[o]);
-    double gxp = 0.0, gxm = 0.0, gyp = 0.0, gym = 0.0, gzp = 0.0, gzm = 0.0;
-    if (!(f & 2)) gxp = (__ldg(&p[row + ((i + 2) & (nx - 1))]) - pc) * r2x;
-    if (!(f & 4)) gxm = (pc - __ldg(&p[row + ((i - 2) & (nx - 1))])) * r2x;
-    if (!(f & 8)) gyp = (__ldg(&p[(size_t)nx * ((size_t)((j + 2) & (ny - 1)) + (size_t)ny * k) + i]) - pc) * r2y;
-    if (!(f & 16)) gym = (pc - __ldg(&p[(size_t)nx * ((size_t)((j - 2) & (ny - 1)) + (size_t)ny * k) + i])) * r2y;
-    if (!(f & 32)) gzp = (__ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k + 2) & (nz - 1))) + i]) - pc) * r2z;
-    if (!(f & 64)) gzm = (pc - __ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k - 2) & (nz - 1))) + i])) * r2z;
-    d[o] = dv + ((gxp - gxm) * r2x + (gyp - gym) * r2y + (gzp - gzm) * r2z);
+#pragma unroll
+    for (int it = 0; it < EQ9_ITEMS; ++it) {
+        const int n = base + it * 256;
+        f[it] = 0x7f;
+        dv[it] = pc[it] = 0.0;
+        if (n < nlist) {
+            f[it] = face[o[it]];
+            dv[it] = FIRST ? d[o[it]] : save[n];
+            pc[it] = __ldg(&p[o[it]]);
+        }
+    }
+#pragma unroll
+    for (int it = 0; it < EQ9_ITEMS; ++it) {
+        const int n = base + it * 256;
+        if (n >= nlist) continue;
+        const uint32_t oo = o[it];
+        const unsigned ff = f[it];
+        const int i = oo & (nx - 1), j = (oo >> lgx) & (ny - 1), k = oo >> (lgx + lgy);
+        if (FIRST) save[n] = dv[it];
+        const size_t row = (size_t)nx * ((size_t)j + (size_t)ny * k);
+        double gxp = 0.0, gxm = 0.0, gyp = 0.0, gym = 0.0, gzp = 0.0, gzm = 0.0;
+        if (!(ff & 2)) gxp = (__ldg(&p[row + ((i + 2) & (nx - 1))]) - pc[it]) * r2x;
+        if (!(ff & 4)) gxm = (pc[it] - __ldg(&p[row + ((i - 2) & (nx - 1))])) * r2x;
+        if (!(ff & 8)) gyp = (__ldg(&p[(size_t)nx * ((size_t)((j + 2) & (ny - 1)) + (size_t)ny * k) + i]) - pc[it]) * r2y;
+        if (!(ff & 16)) gym = (pc[it] - __ldg(&p[(size_t)nx * ((size_t)((j - 2) & (ny - 1)) + (size_t)ny * k) + i])) * r2y;
+        if (!(ff & 32)) gzp = (__ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k + 2) & (nz - 1))) + i]) - pc[it]) * r2z;
+        if (!(ff & 64)) gzm = (pc[it] - __ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k - 2) & (nz - 1))) + i])) * r2z;
+        d[oo] = dv[it] + ((gxp - gxm) * r2x + (gyp - gym) * r2y + (gzp - gzm) * r2z);
+    }
 }
 
 // NEXT-1, eq. 6: out = beta ? f + sum_a gamma_a d6_a f : +0.0 with gamma_a = Delta_a^6/pi^6 and
