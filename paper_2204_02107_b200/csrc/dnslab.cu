@@ -114,6 +114,7 @@ struct dnslab {
     int st_rev;  // bit per stencil kernel of a step (RK stages 1-4, divergence, projection): same idea
     int fft_rev; // bit per pass of a solve (x fwd, y fwd, z, y inv, x inv): walk its tiles from the far end
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
+    int pair_mode; // 0: stages 1+2 and 3+4 fused; 1: only stages 1+2 fused (env DNSLAB_PAIR_MODE)
     int pair_kc; // > 0: two-stage kernel (k_rk_pair) with this many planes per block; 0: one launch per stage
     // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
     bool prof_on;
@@ -621,6 +622,8 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
         }
         // two stages per launch (flags bit 3) for nx >= 32, ny >= 16: one block per SM, >= 6 waves, at least 8 planes each
         h->pair_kc = 0;
+        h->pair_mode = 0;
+        if (const char *v = getenv("DNSLAB_PAIR_MODE")) h->pair_mode = atoi(v);
         if (params->nx >= dnsst::P2_TX && params->ny >= dnsst::P2_TY && ((params->flags & 8u) || getenv("DNSLAB_RK_PAIR"))) {
             const long tiles = (long)(params->nx / dnsst::P2_TX) * (params->ny / dnsst::P2_TY);
             int kc = params->nz;
@@ -762,8 +765,13 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
     const size_t bytes = h->n * sizeof(double);
     int rc;
     for (int it = 0; it < nsteps; ++it) {
-        if (!stage_proj && h->pair_kc > 0) {
-            // two launches: stages 1+2 (A = Q2, Bf = Q3), stages 3+4 (Q4 stays on chip, Q* overwrites A)
+        if (!stage_proj && h->pair_kc > 0 && h->pair_mode == 1) {
+            // stages 1+2 in one launch (Q2 stays on chip; Bf = Q3, Qc = S), then stages 3 and 4 as single launches
+            if ((rc = launch_rk_pair<0>(h, h->Q, h->Qc, h->Bf))) return rc;
+            if ((rc = launch_rk<3, true>(h, h->Bf, h->A, nullptr, nullptr))) return rc;
+            if ((rc = launch_rk<4, true>(h, h->A, nullptr, h->Qc, nullptr))) return rc;
+        } else if (!stage_proj && h->pair_kc > 0) {
+            // two launches: stages 1+2 (A = S, Bf = Q3), stages 3+4 (Q4 stays on chip, Q* overwrites A)
             if ((rc = launch_rk_pair<0>(h, h->Q, h->A, h->Bf))) return rc;
             if ((rc = launch_rk_pair<1>(h, h->Bf, h->A, h->Bf))) return rc;
         } else if (!stage_proj) {
@@ -775,7 +783,8 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
         }
         if (!stage_proj) {
             // Q* is in A (two-stage kernels) or Qc (one kernel per stage); the other one is free for the filter
-            double **fin = h->pair_kc > 0 ? h->A : h->Qc, **spare = h->pair_kc > 0 ? h->Qc : h->A;
+            const bool inA = h->pair_kc > 0 && h->pair_mode != 1;
+            double **fin = inA ? h->A : h->Qc, **spare = inA ? h->Qc : h->A;
             if ((rc = pressure_stage(h, fin, h->p))) return rc;
             if (filter) {
                 if ((rc = launch_filter(h, fin, spare))) return rc;
