@@ -61,6 +61,10 @@ typedef struct {
     double *q[4];            /* u, v, w, c  (state Q^n) */
     double *p;               /* pressure (state: warm start of eq. 9) */
     double *qs[4], *qc[4], *f[4], *d, *r, *re, *im;
+    /* NEXT-4: Lagrangian particles attached by the caller (state lives in the caller's array) */
+    int64_t np;
+    double *part; /* 8 arrays of np doubles: x, y, z, u, v, w, d, rho_p */
+    double rho_f, grav[3];
 } dnsref_t;
 
 int dnsref_num_threads(void)
@@ -397,6 +401,8 @@ static void pressure_stage(dnsref_t *h, double *us, double *vs, double *ws, doub
     dnsref_project(h, us, vs, ws, p, us, vs, ws);
 }
 
+int dnsref_particles_step(const dnsref_t *h, int64_t n, double *state, double rho_f, const double g[3]);
+
 /* ------------------------------------------------------------------------
  * One full time step (PAPER.md:43 RK4 + projection once per step):
  *   Qc = Qn; Qs = Qn
@@ -439,7 +445,77 @@ int dnsref_step(dnsref_t *h, int nsteps)
             if (h->P.flags & 1u) dnsref_filter(h, h->qc[m], h->q[m]); /* eq. 6, end of step (NEXT-1) */
             else memcpy(h->q[m], h->qc[m], sizeof(double) * n);
         }
+        if (h->np > 0) dnsref_particles_step(h, h->np, h->part, h->rho_f, h->grav); /* NEXT-4, after the fluid step */
     }
+    return DNSREF_OK;
+}
+
+/* ------------------------------------------------------------------------
+ * NEXT-4: Lagrangian particles, eqs. 10-13, advanced by one fluid time step dt with
+ * the velocity field given (the paper's "SolveDrops.m" runs after the fluid step):
+ *     tau_p = rho_p d^2 / (18 rho_f nu)                                   (eq. 11; d enters as in Stokes' law)
+ *     Re_p  = |u_f - u_p| d / nu,   C_d = 1 + Re_p^(2/3) / 6              (eqs. 12, 13)
+ *     du_p/dt = (C_d / tau_p)(u_f - u_p) + g                              (eq. 10)
+ * "solved using the implicit Euler method".  Readings (R26-R28): u_f is the
+ * trilinear interpolation of the collocated velocity (cell centres at x_i = i Delta, periodic); C_d is
+ * evaluated with the velocities at the old time level, the drag term is implicit in u_p:
+ *     u_p' = (u_p + dt (k u_f + g)) / (1 + dt k),  k = C_d / tau_p;       x_p' = x_p + dt u_p'  (wrapped into [0, L)).
+ * state: 8 arrays of n doubles, x y z u v w d rho_p.  Solid cells hold u = 0 and take part in the
+ * interpolation like any other cell; there is no deposition model in the paper.
+ * ---------------------------------------------------------------------- */
+static double interp3(const dnsref_t *h, const double *f, double x, double y, double z)
+{
+    const int nx = h->P.nx, ny = h->P.ny, nz = h->P.nz;
+    const double gx = x / h->P.dx, gy = y / h->P.dy, gz = z / h->P.dz;
+    const double fx = floor(gx), fy = floor(gy), fz = floor(gz);
+    const double ax = gx - fx, ay = gy - fy, az = gz - fz;
+    const int i0 = wrapm((int)fx, nx), j0 = wrapm((int)fy, ny), k0 = wrapm((int)fz, nz);
+    const int i1 = wrapm(i0 + 1, nx), j1 = wrapm(j0 + 1, ny), k1 = wrapm(k0 + 1, nz);
+    const double c00 = f[IDX(i0, j0, k0)] * (1.0 - ax) + f[IDX(i1, j0, k0)] * ax;
+    const double c10 = f[IDX(i0, j1, k0)] * (1.0 - ax) + f[IDX(i1, j1, k0)] * ax;
+    const double c01 = f[IDX(i0, j0, k1)] * (1.0 - ax) + f[IDX(i1, j0, k1)] * ax;
+    const double c11 = f[IDX(i0, j1, k1)] * (1.0 - ax) + f[IDX(i1, j1, k1)] * ax;
+    const double c0 = c00 * (1.0 - ay) + c10 * ay, c1 = c01 * (1.0 - ay) + c11 * ay;
+    return c0 * (1.0 - az) + c1 * az;
+}
+
+int dnsref_particles_step(const dnsref_t *h, int64_t n, double *state, double rho_f, const double g[3])
+{
+    if (!h || n < 0 || (n > 0 && !state) || !g || !(rho_f > 0) || !(h->P.nu > 0)) return DNSREF_EINVAL;
+    double *px = state, *py = state + n, *pz = state + 2 * n, *pu = state + 3 * n, *pv = state + 4 * n, *pw = state + 5 * n;
+    const double *pd = state + 6 * n, *pr = state + 7 * n;
+    const double dt = h->P.dt, nu = h->P.nu;
+    const double len[3] = {h->P.nx * h->P.dx, h->P.ny * h->P.dy, h->P.nz * h->P.dz};
+    for (int64_t q = 0; q < n; ++q) {
+        const double uf = interp3(h, h->q[0], px[q], py[q], pz[q]);
+        const double vf = interp3(h, h->q[1], px[q], py[q], pz[q]);
+        const double wf = interp3(h, h->q[2], px[q], py[q], pz[q]);
+        const double tau = pr[q] * pd[q] * pd[q] / (18.0 * rho_f * nu);
+        const double rel = sqrt((uf - pu[q]) * (uf - pu[q]) + (vf - pv[q]) * (vf - pv[q]) + (wf - pw[q]) * (wf - pw[q]));
+        const double rep = rel * pd[q] / nu;
+        const double cd = 1.0 + cbrt(rep * rep) / 6.0;
+        const double k = cd / tau;
+        pu[q] = (pu[q] + dt * (k * uf + g[0])) / (1.0 + dt * k);
+        pv[q] = (pv[q] + dt * (k * vf + g[1])) / (1.0 + dt * k);
+        pw[q] = (pw[q] + dt * (k * wf + g[2])) / (1.0 + dt * k);
+        double xn[3] = {px[q] + dt * pu[q], py[q] + dt * pv[q], pz[q] + dt * pw[q]};
+        for (int a = 0; a < 3; ++a) {
+            xn[a] = xn[a] - floor(xn[a] / len[a]) * len[a];
+            if (!(xn[a] < len[a])) xn[a] = 0.0; /* rounding at the upper edge */
+        }
+        px[q] = xn[0]; py[q] = xn[1]; pz[q] = xn[2];
+    }
+    return DNSREF_OK;
+}
+
+/* Particles to be advanced at the end of every dnsref_step (n = 0 detaches); the array stays the caller's. */
+int dnsref_particles_attach(dnsref_t *h, int64_t n, double *state, double rho_f, const double g[3])
+{
+    if (!h || n < 0) return DNSREF_EINVAL;
+    if (n > 0 && (!state || !g || !(rho_f > 0) || !(h->P.nu > 0))) return DNSREF_EINVAL;
+    h->np = n;
+    h->part = n > 0 ? state : NULL;
+    if (n > 0) { h->rho_f = rho_f; h->grav[0] = g[0]; h->grav[1] = g[1]; h->grav[2] = g[2]; }
     return DNSREF_OK;
 }
 

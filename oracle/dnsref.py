@@ -57,6 +57,8 @@ def lib():
         L.dnsref_div.restype = None
         L.dnsref_poisson_rhs.argtypes = [C.c_void_p] + [C.c_void_p] * 3
         L.dnsref_poisson_rhs.restype = None
+        L.dnsref_particles_step.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_double, C.POINTER(C.c_double)]
+        L.dnsref_particles_attach.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.dnsref_courant.argtypes = [C.c_void_p]
         L.dnsref_courant.restype = C.c_double
         L.dnsref_set_dt.argtypes = [C.c_void_p, C.c_double]
@@ -185,6 +187,27 @@ class Oracle:
         r = self._new()
         lib().dnsref_poisson_rhs(self._h, _ptr(d), _ptr(p), _ptr(r))
         return r
+
+    def particles_step(self, state, rho_f, g):
+        """One particle step (eqs. 10-13) in the current velocity field; state: float64 (8, n) rows x y z u v w d rho_p,
+        updated in place."""
+        assert state.dtype == np.float64 and state.ndim == 2 and state.shape[0] == 8 and state.flags.c_contiguous
+        gg = (C.c_double * 3)(*[float(x) for x in g])
+        rc = lib().dnsref_particles_step(self._h, state.shape[1], _ptr(state), float(rho_f), gg)
+        if rc:
+            raise ValueError("dnsref_particles_step")
+
+    def particles_attach(self, state, rho_f=1.2, g=(0.0, 0.0, 0.0)):
+        """Advance these particles at the end of every step (state is kept and updated in place); None detaches."""
+        gg = (C.c_double * 3)(*[float(x) for x in g])
+        if state is None:
+            rc = lib().dnsref_particles_attach(self._h, 0, None, 1.0, gg)
+        else:
+            assert state.dtype == np.float64 and state.ndim == 2 and state.shape[0] == 8 and state.flags.c_contiguous
+            rc = lib().dnsref_particles_attach(self._h, state.shape[1], _ptr(state), float(rho_f), gg)
+        self._particles = state
+        if rc:
+            raise ValueError("dnsref_particles_attach")
 
     def courant(self):
         """dt * max_cells(|u|/dx + |v|/dy + |w|/dz) of the current state (reading R24)."""

@@ -589,3 +589,90 @@ def test_P16_scalar_stats_closed_form_library_and_mask():
     solid = mk(shape, mask=np.zeros(shape, np.uint8))
     solid.set_fields(z, z, z, c)
     assert solid.scalar_stats((0, 0, 0), (4, 4, 4)) == (0.0, 0.0, 0)
+
+
+# ---------------------------------------------------------------- Lagrangian particles (P17, NEXT-4)
+def _particles(rows):
+    return np.ascontiguousarray(np.array(rows, dtype=np.float64).T)          # (8, n): x y z u v w d rho_p
+
+
+def test_P17_sedimentation_times_printed_in_the_paper():
+    """Quiescent air: the settling velocity reached by the implicit Euler steps gives tau_s = h/v for h = 1.5 m of
+    36/9/1 min for d = 5/10/30 um (tests/golden/sedimentation.txt) at the paper's rounding; the
+    steady state satisfies eq. 10 with du_p/dt = 0:  (C_d/tau_p)(0 - w) + g = 0."""
+    rows = [l.split() for l in open(os.path.join(GOLD, "sedimentation.txt")) if l.strip() and not l.startswith("#")]
+    nu, rho_f, rho_p, g = 1.6e-5, 1.2, 1000.0, -9.81
+    o = mk((8, 8, 8), (0.25, 0.25, 0.25), nu=nu, dt=0.05)            # dt >> tau_p: implicit Euler stays stable
+    z = np.zeros((8, 8, 8))
+    o.set_fields(z, z, z, z)
+    st = _particles([[1.0, 1.0, 1.0, 0.0, 0.0, 0.0, float(d) * 1e-6, rho_p] for d, _ in rows])
+    for _ in range(40):
+        o.particles_step(st, rho_f, (0.0, 0.0, g))
+    for q, (d, minutes) in enumerate(rows):
+        d_m, w = float(d) * 1e-6, st[5, q]
+        tau_p = rho_p * d_m ** 2 / (18 * rho_f * nu)
+        cd = 1 + (abs(w) * d_m / nu) ** (2.0 / 3.0) / 6
+        assert abs(cd / tau_p * (0.0 - w) + g) <= 1e-9 * abs(g)                     # fixed point of eq. 10
+        tau_s_min = 1.5 / abs(w) / 60.0
+        assert abs(tau_s_min - float(minutes)) <= 0.06 * float(minutes) + 0.05, (d, tau_s_min)
+        assert st[3, q] == 0.0 and st[4, q] == 0.0
+
+
+def test_P17_implicit_euler_is_bounded_and_unconditionally_stable():
+    """From rest in still air |w| stays within [0, g tau_p] (C_d >= 1) and settles on the fixed point of eq. 10 for
+    dt from 0.01 tau_p to 1e4 tau_p (C_d is lagged, reading R27, so the approach may overshoot the fixed point a
+    little, but never the Stokes velocity)."""
+    nu, rho_f, rho_p, d = 1.6e-5, 1.2, 1000.0, 30e-6
+    tau_p = rho_p * d * d / (18 * rho_f * nu)
+    for fac, nsteps in ((0.01, 3000), (1.0, 60), (1e4, 30)):
+        o = mk((8, 8, 8), (1.0, 1.0, 1.0), nu=nu, dt=fac * tau_p)
+        z = np.zeros((8, 8, 8))
+        o.set_fields(z, z, z, z)
+        st = _particles([[4.0, 4.0, 4.0, 0, 0, 0, d, rho_p]])
+        for _ in range(nsteps):
+            o.particles_step(st, rho_f, (0, 0, -9.81))
+            assert 0.0 <= -st[5, 0] <= 9.81 * tau_p
+        w = st[5, 0]
+        cd = 1 + (abs(w) * d / nu) ** (2.0 / 3.0) / 6
+        assert abs(cd / tau_p * (0.0 - w) - 9.81) <= 1e-6 * 9.81, fac
+
+
+def test_P17_trilinear_interpolation_at_nodes_midpoints_and_across_the_seam():
+    """A very light particle (dt C_d/tau_p ~ 1e12) takes the interpolated fluid velocity in one step: node value at a
+    node, two-point mean at an edge midpoint (also across the periodic seam), eight-point mean at a cell centre;
+    the position moves by dt u_p and wraps into [0, L)."""
+    rng_ = np.random.default_rng(17)
+    shape, d = (8, 8, 8), (0.5, 0.25, 0.2)
+    u, v, w = (rng_.standard_normal(shape) for _ in range(3))
+    o = mk(shape, d, nu=1.0, dt=1e-3)
+    o.set_fields(u, v, w, np.zeros(shape))
+    pts = [((3, 2, 1), [(3, 2, 1)]), ((3.5, 2, 1), [(3, 2, 1), (4, 2, 1)]), ((7.5, 0, 0), [(7, 0, 0), (0, 0, 0)]),
+           ((2, 7.5, 3), [(2, 7, 3), (2, 0, 3)]), ((1, 1, 7.5), [(1, 1, 7), (1, 1, 0)]),
+           ((1.5, 2.5, 3.5), [(a, b, c) for a in (1, 2) for b in (2, 3) for c in (3, 4)])]
+    st = _particles([[p[0] * d[0], p[1] * d[1], p[2] * d[2], 0, 0, 0, 1e-9, 1.0] for p, _ in pts])
+    x0 = st[:3].copy()
+    o.particles_step(st, 1.0, (0, 0, 0))
+    L = np.array([8 * d[0], 8 * d[1], 8 * d[2]])
+    for q, (_, cells) in enumerate(pts):
+        for comp, f in enumerate((u, v, w)):
+            want = np.mean([f[c[2], c[1], c[0]] for c in cells])
+            assert abs(st[3 + comp, q] - want) <= 1e-11 * max(1.0, abs(want)), (q, comp)
+        xn = (x0[:, q] + 1e-3 * st[3:6, q]) % L
+        assert np.abs(st[:3, q] - xn).max() <= 1e-14 and np.all(st[:3, q] >= 0) and np.all(st[:3, q] < L)
+
+
+def test_P17_attached_particles_follow_the_stepped_field():
+    """attach: the particle step runs after each fluid step with the NEW field -- equal to stepping by hand."""
+    case = cases.taylor_green(16)
+    kw = dict(nu=case["nu"], alpha_c=case["alpha_c"], dt=case["dt"], n_piter=1)
+    a, b = mk(case["shape"], case["d"], **kw), mk(case["shape"], case["d"], **kw)
+    for o in (a, b):
+        o.set_fields(case["u"], case["v"], case["w"], case["c"])
+    st_a = _particles([[1.0, 2.0, 3.0, 0, 0, 0, 1e-3, 1000.0], [5.0, 0.1, 6.2, 0.1, 0, 0, 2e-3, 500.0]])
+    st_b = st_a.copy()
+    a.particles_attach(st_a, 1.2, (0, 0, -9.81))
+    a.step(3)
+    for _ in range(3):
+        b.step(1)
+        b.particles_step(st_b, 1.2, (0, 0, -9.81))
+    assert np.array_equal(st_a, st_b) and not np.array_equal(st_a[:3], _particles([[1.0, 2.0, 3.0, 0, 0, 0, 1e-3, 1000.0]])[:3])
