@@ -127,7 +127,8 @@ int64_t dnslab_launch_count(const dnslab_t *h);
 #define DNSLAB_K_EQ9 6     /* eq. 9 right-hand side at the cells next to solid cells       */
 #define DNSLAB_K_FILTER 7  /* eq. 6 filter (flags bit 0)                                    */
 #define DNSLAB_K_REDUCE 8  /* Courant-number and scalar mean/std reductions (NEXT-3)         */
-#define DNSLAB_NCLASS 9
+#define DNSLAB_K_PARTICLES 9 /* Lagrangian particle step (NEXT-4)                             */
+#define DNSLAB_NCLASS 10
 int dnslab_profile(dnslab_t *h, int enable);
 int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches);
 
@@ -145,6 +146,17 @@ int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches);
 int dnslab_courant(dnslab_t *h, double *co);
 int dnslab_set_dt(dnslab_t *h, double dt);
 int dnslab_scalar_stats(dnslab_t *h, const int32_t lo[3], const int32_t size[3], double out[3]);
+
+/* ---- NEXT-4: Lagrangian particles, eqs. 10-13 ------------------------------------------
+ * dnslab_particles_attach: from now on every time step of dnslab_step ends with one implicit Euler step of size
+ * dt of the n particles in `state`, in the velocity field just computed (the paper's "SolveDrops.m" after the
+ * fluid solve).  state is DEVICE memory owned by the caller, 8 arrays of n doubles one after the
+ * other: x, y, z (positions in [0, N_a Delta_a), cell centres at i Delta), u, v, w (particle velocity),
+ * d (diameter as it enters eq. 11), rho_p; the first six are updated in place.  rho_f > 0 is the fluid density of
+ * eq. 11, g[3] the gravitational acceleration of eq. 10 (host pointer, copied).  u_f is the trilinear interpolation
+ * of u, v, w (R26), C_d is taken from the old velocities (R27), positions wrap periodically (R28).
+ * n = 0 detaches.  DNSLAB_EINVAL for n < 0, a null state with n > 0, rho_f <= 0, or nu = 0 (eq. 11 divides by it). */
+int dnslab_particles_attach(dnslab_t *h, int64_t n, double *state, double rho_f, const double g[3]);
 
 int dnslab_destroy(dnslab_t *h);
 

@@ -12,8 +12,8 @@ LIB_PATH = os.path.join(_HERE, "libdnslab.so")
 
 SYMBOLS = ["dnslab_workspace_bytes", "dnslab_create", "dnslab_set_fields", "dnslab_step", "dnslab_poisson",
            "dnslab_fields", "dnslab_get_fields", "dnslab_launch_count", "dnslab_profile", "dnslab_profile_read",
-           "dnslab_courant", "dnslab_set_dt", "dnslab_scalar_stats", "dnslab_destroy", "dnslab_strerror"]
-KERNEL_CLASSES = ["rk_stage", "div", "fft_x", "fft_y", "fft_z_solve", "project", "eq9_sparse", "filter", "reduce"]
+           "dnslab_courant", "dnslab_set_dt", "dnslab_scalar_stats", "dnslab_particles_attach", "dnslab_destroy", "dnslab_strerror"]
+KERNEL_CLASSES = ["rk_stage", "div", "fft_x", "fft_y", "fft_z_solve", "project", "eq9_sparse", "filter", "reduce", "particles"]
 
 
 class Params(C.Structure):
@@ -60,6 +60,7 @@ def lib():
         L.dnslab_courant.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.dnslab_set_dt.argtypes = [C.c_void_p, C.c_double]
         L.dnslab_scalar_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_double)]
+        L.dnslab_particles_attach.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.dnslab_destroy.argtypes = [C.c_void_p]
         L.dnslab_strerror.argtypes = [C.c_int]
         L.dnslab_strerror.restype = C.c_char_p
@@ -170,6 +171,18 @@ class Solver:
 
     def launch_count(self):
         return int(lib().dnslab_launch_count(self._h))
+
+    def particles_attach(self, state, rho_f=1.2, g=(0.0, 0.0, 0.0)):
+        """dnslab_particles_attach: state is a contiguous float64 CUDA tensor of shape (8, n) (rows x y z u v w d rho_p),
+        advanced in place at the end of every step; None detaches.  The caller keeps the tensor alive."""
+        gg = (C.c_double * 3)(*[float(x) for x in g])
+        if state is None:
+            _check(lib().dnslab_particles_attach(self._h, 0, None, 1.0, gg), "dnslab_particles_attach")
+        else:
+            assert state.is_cuda and state.is_contiguous() and state.dim() == 2 and state.shape[0] == 8
+            _check(lib().dnslab_particles_attach(self._h, int(state.shape[1]), state.data_ptr(), float(rho_f), gg),
+                   "dnslab_particles_attach")
+        self._particles = state
 
     def courant(self):
         """dnslab_courant: dt * max_cells(|u|/dx + |v|/dy + |w|/dz); synchronises."""

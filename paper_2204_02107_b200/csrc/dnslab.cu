@@ -11,6 +11,7 @@
 
 #include "../../include/dnslab.h"
 #include "fft.cuh"
+#include "particles.cuh"
 #include "reduce.cuh"
 #include "stencil.cuh"
 
@@ -114,6 +115,8 @@ struct dnslab {
     int st_rev;  // bit per stencil kernel of a step (RK stages 1-4, divergence, projection): same idea
     int fft_rev; // bit per pass of a solve (x fwd, y fwd, z, y inv, x inv): walk its tiles from the far end
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
+    long long np;      // NEXT-4: attached particles (0: none); state is the caller's device array
+    double *pstate, prho_f, pgrav[3];
     int pair_mode; // 0: stages 1+2 and 3+4 fused; 1: only stages 1+2 fused (env DNSLAB_PAIR_MODE)
     int pair_kc; // > 0: two-stage kernel (k_rk_pair) with this many planes per block; 0: one launch per stage
     // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
@@ -530,6 +533,22 @@ int launch_filter(dnslab *h, double *const *in, double *const *out)
     return check_launch(h);
 }
 
+// NEXT-4: one implicit Euler step of the attached particles in the field h->Q
+int launch_particles(dnslab *h)
+{
+    dnspart::PartArgs a;
+    a.u = h->Q[0]; a.v = h->Q[1]; a.w = h->Q[2];
+    a.state = h->pstate;
+    a.n = h->np;
+    a.nx = h->P.nx; a.ny = h->P.ny; a.nz = h->P.nz;
+    a.dx = h->P.dx; a.dy = h->P.dy; a.dz = h->P.dz;
+    a.dt = h->P.dt; a.nu = h->P.nu; a.rho_f = h->prho_f;
+    for (int c = 0; c < 3; ++c) a.g[c] = h->pgrav[c];
+    ProfScope ps(h, DNSLAB_K_PARTICLES);
+    dnspart::k_particles<<<(unsigned)((h->np + 127) / 128), 128, 0, h->stream>>>(a);
+    return check_launch(h);
+}
+
 // divergence, n_piter iterations of eq. 9 warm-started from p, correction (in place on q)
 int pressure_stage(dnslab *h, double *const *q, double *p)
 {
@@ -795,6 +814,7 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
                 h->Q[m] = fin[m];
                 fin[m] = t;
             }
+            if (h->np > 0 && (rc = launch_particles(h))) return rc;
             continue;
         }
         // NEXT-2 variant: every stage field is projected, so the accumulate form is needed
@@ -819,6 +839,7 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
             h->Q[m] = fin[m];
             fin[m] = t;
         }
+        if (h->np > 0 && (rc = launch_particles(h))) return rc;
     }
     return DNSLAB_OK;
 }
@@ -875,6 +896,19 @@ int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches)
     for (int c = 0; c < DNSLAB_NCLASS; ++c) {
         ms[c] = h->prof_ms[c];
         launches[c] = h->prof_n[c];
+    }
+    return DNSLAB_OK;
+}
+
+int dnslab_particles_attach(dnslab_t *h, int64_t n, double *state, double rho_f, const double g[3])
+{
+    if (!h || n < 0) return DNSLAB_EINVAL;
+    if (n > 0 && (!state || !g || !(rho_f > 0) || !(h->P.nu > 0))) return DNSLAB_EINVAL;
+    h->np = n;
+    h->pstate = n > 0 ? state : nullptr;
+    if (n > 0) {
+        h->prho_f = rho_f;
+        for (int c = 0; c < 3; ++c) h->pgrav[c] = g[c];
     }
     return DNSLAB_OK;
 }

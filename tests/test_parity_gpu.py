@@ -192,6 +192,58 @@ def test_next3_courant_set_dt_and_scalar_stats():
     s.close()
 
 
+def test_next4_lagrangian_particles():
+    """NEXT-4: particles attached to the solver are advanced after every fluid step (eqs. 10-13, implicit Euler);
+    positions and velocities match the oracle's after 1 and 20 steps in a masked room (5-100 um droplets under gravity)
+    and in a periodic box with order-one velocities (positions wrap through the seam); 100 000 particles for one step
+    span many blocks; detaching stops the updates."""
+    import torch
+
+    def seed_particles(case, n, seed, dmin, dmax):
+        r = np.random.default_rng(seed)
+        nz, ny, nx = case["shape"]
+        L = np.array([nx * case["d"][0], ny * case["d"][1], nz * case["d"][2]])
+        st = np.empty((8, n))
+        st[0:3] = r.random((3, n)) * L[:, None]
+        st[0, : min(n, 4)] = [0.0, L[0] * (1 - 1e-12), 0.5 * case["d"][0], L[0] - 0.5 * case["d"][0]][: min(n, 4)]   # on and next to the seam
+        st[3:6] = 0.01 * r.standard_normal((3, n))
+        st[6] = dmin + (dmax - dmin) * r.random(n)
+        st[7] = 1000.0
+        return st, L
+
+    for case, n, cps, dmin, dmax, g in [(cases.duct_room(64, 32, 32), 257, [1, 20], 5e-6, 100e-6, (0.0, 0.0, -9.81)),
+                                        (cases.periodic_turbulence(32, steps=5), 1000, [1, 5], 1e-3, 2e-2, (0.0, 0.0, 0.0)),
+                                        (cases.duct_room(32, 16, 16), 100000, [1], 5e-6, 100e-6, (0.0, 0.0, -9.81))]:
+        st0, L = seed_particles(case, n, 44, dmin, dmax)
+        s = binding.solver_for_case(case)
+        o = oracle_for(case)
+        dev = torch.from_numpy(st0.copy()).cuda()
+        host = st0.copy()
+        s.particles_attach(dev, 1.2, g)
+        o.particles_attach(host, 1.2, g)
+        done = 0
+        for cp in cps:
+            s.step(cp - done)
+            o.step(cp - done)
+            done = cp
+            got = dev.cpu().numpy()
+            tol = TOL1 if cp == 1 else TOL100
+            dx = np.abs(got[0:3] - host[0:3])
+            dx = np.minimum(dx, L[:, None] - dx)                      # a particle on the seam may land on either side
+            assert (dx / L[:, None]).max() <= tol, (case["name"], cp, (dx / L[:, None]).max())
+            vs = max(np.abs(host[3:6]).max(), 1e-300)
+            assert np.abs(got[3:6] - host[3:6]).max() / vs <= tol, (case["name"], cp)
+            assert np.array_equal(got[6:8], st0[6:8])
+            assert np.all(got[0:3] >= 0) and np.all(got[0:3] < L[:, None])
+        compare(s.fields_numpy(), o.fields(), TOL100, mask=case["mask"], what="fields untouched by particles")
+        assert not np.array_equal(dev.cpu().numpy()[0:3], st0[0:3])
+        s.particles_attach(None)
+        before = dev.clone()
+        s.step(1)
+        assert torch.equal(before, dev)
+        s.close()
+
+
 def test_two_stage_rk_kernel_variant():
     """flags bit 3: stages 1+2 and 3+4 fused (k_rk_pair, intermediate stage field in shared memory) -- same method,
     same tolerances; masked with sources, unmasked, a grid of one tile in x, and a z extent of one chunk."""
