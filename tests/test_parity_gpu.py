@@ -131,6 +131,15 @@ def test_config4_full_size_one_step():
         compare(got, ref, TOL1, mask=case["mask"], what="room512 step 1")
 
 
+@pytest.mark.slow
+def test_config5_half_size_one_step():
+    """Config 5's generator (three rooms, doorways, two ducts, 30 boxes) at 512x256x128 -- the largest size at which the
+    oracle still finishes a step in seconds (full size: 134 M cells, 22 GB and minutes per oracle step)."""
+    case = cases.config(5, shrink=2)
+    for cp, got, ref in run_both(case, [1]):
+        compare(got, ref, TOL1, mask=case["mask"], what="rooms/2 step 1")
+
+
 # ------------------------------------------------------------------ variants and edge cases
 def test_per_stage_projection_variant():
     case = cases.duct_room(32, 16, 16)
