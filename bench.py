@@ -295,7 +295,10 @@ def run_ours(args):
                          "bytes_per_cell_per_launch": cb[dom], "share_of_step": d_ms / tot_ms,
                          "moved_bytes_per_cell_per_launch": mv[dom], "achieved_moved": achieved_moved,
                          "frac_moved": achieved_moved / peak, "near_solid_fraction": fb,
-                         "timing": "CUDA events around every launch (dnslab_profile), separate pass of K steps"},
+                         "timing": "CUDA events around every launch (dnslab_profile), separate pass of K steps",
+                         "note": "achieved/frac count SURVEY.md 8(d)'s canonical bytes (the fixed denominator; 65 RK field passes "
+                                 "per step); this implementation moves fewer (48), so frac can exceed 1 -- achieved_moved/"
+                                 "frac_moved count the bytes it really moves, and traffic is ncu's DRAM bytes per launch"},
             "step_roofline": {"canonical_bytes_per_cell": canonical_bytes_per_cell(P, masked), "achieved": step_gbs,
                               "peak": peak, "unit": "GB/s", "frac": step_gbs / peak},
             "kernels": breakdown,
