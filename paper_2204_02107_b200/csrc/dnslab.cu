@@ -112,6 +112,7 @@ struct dnslab {
     int64_t launches;
     dim3 rk_block;
     int nsm;   // SM count of the device
+    int z_oneshot; // fused z pass: one tile per block instead of the persistent kernel (env DNSLAB_Z_ONESHOT)
     int st_rev;  // bit per stencil kernel of a step (RK stages 1-4, divergence, projection): same idea
     int fft_rev; // bit per pass of a solve (x fwd, y fwd, z, y inv, x inv): walk its tiles from the far end
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
@@ -392,6 +393,15 @@ template <int L, int XT> int launch_fft_z_solve_LX(dnslab *h, c2 *data)
     const int mx = h->P.nx / 2;
     const size_t smem = 2 * (size_t)XT * L * sizeof(c2);
     const size_t ntiles = (size_t)(mx / XT) * h->P.ny;
+    if (h->z_oneshot) {
+        const size_t smem1 = (size_t)XT * L * sizeof(c2);
+        auto kern1 = dnsfft::k_fft_z_solve1<L, XT>;
+        if (smem1 > 48 * 1024) CK(cudaFuncSetAttribute(kern1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
+        ProfScope ps(h, DNSLAB_K_FFT_Z);
+        kern1<<<(unsigned)ntiles, XT * T, smem1, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2],
+                                                              2.0 / (double)h->n, (h->fft_rev >> 2) & 1);
+        return check_launch(h);
+    }
     auto kern = dnsfft::k_fft_z_solve<L, XT>;
     unsigned grid = 0;
     if (int rc = persistent_grid(h, kern, NT, smem, ntiles, &grid)) return rc;
@@ -604,6 +614,7 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
     h->nsm = prop.multiProcessorCount;
     h->fft_rev = 10; // y passes walk against the x passes: 41.7 instead of 45 us each (measured sweep over the 5-bit choices)
     if (const char *v = getenv("DNSLAB_FFT_REV")) h->fft_rev = atoi(v);
+    h->z_oneshot = getenv("DNSLAB_Z_ONESHOT") ? atoi(getenv("DNSLAB_Z_ONESHOT")) : 0;
     h->st_rev = 16; // only the divergence gains from it (83 instead of 88 us); the RK stages do not
     if (const char *v = getenv("DNSLAB_ST_REV")) h->st_rev = atoi(v);
     h->ws = (char *)workspace;
