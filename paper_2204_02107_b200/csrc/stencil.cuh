@@ -267,11 +267,16 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
     issue_plane(k0, 0);
     issue_plane(k0 + 1, 1);
     issue_plane(k0 + 2, 2);
-    double2 zm[4], cur[4];
+    // z-carried values of this thread's column: three register sets that take the roles z-1, centre, z+1 in
+    // turn (the plane loop is unrolled three times, so the carry is a renaming, not a copy)
+    double2 r0[4], r1[4], r2[4];
     {
         const size_t pkm = plane * (size_t)((k0 - 1) & (nz - 1));
 #pragma unroll
-        for (int m = 0; m < 4; ++m) zm[m] = __ldg(reinterpret_cast<const double2 *>(a.qs[m] + pkm + orow));
+        for (int m = 0; m < 4; ++m) {
+            r0[m] = __ldg(reinterpret_cast<const double2 *>(a.qs[m] + pkm + orow));
+            r1[m] = r2[m] = make_double2(0.0, 0.0);
+        }
     }
     const int own = (ty + 1) * SW + 2 + 2 * tx; // this thread's pair inside a field's tile
     unsigned fraw_next = 0x7f7f;
@@ -286,7 +291,7 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
         }
     }
 
-    for (int t = 0; t < kc; ++t) {
+    auto plane_step = [&](const int t, double2 (&zm)[4], double2 (&cur)[4], double2 (&zp)[4]) {
         const int k = k0 + t;
         const size_t o = plane * (size_t)k + orow;
         // operands that do not go through shared memory: issue their loads before waiting
@@ -310,7 +315,6 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
 #pragma unroll
             for (int m = 0; m < 4; ++m) cur[m] = *reinterpret_cast<const double2 *>(sC + m * ROWS * SW + own);
         }
-        double2 zp[4];
 #pragma unroll
         for (int m = 0; m < 4; ++m) zp[m] = *reinterpret_cast<const double2 *>(sN + m * ROWS * SW + own);
         if (STAGE == 1) {
@@ -441,11 +445,13 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
                 }
             }
         }
-#pragma unroll
-        for (int m = 0; m < 4; ++m) {
-            zm[m] = cur[m];
-            cur[m] = zp[m];
-        }
+    };
+    for (int t = 0; t < kc; t += 3) {
+        plane_step(t, r0, r1, r2);
+        if (t + 1 >= kc) break;
+        plane_step(t + 1, r1, r2, r0);
+        if (t + 2 >= kc) break;
+        plane_step(t + 2, r2, r0, r1);
     }
 }
 
