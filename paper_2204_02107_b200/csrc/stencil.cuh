@@ -189,7 +189,7 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
 // (plus the one-cell halo), the bytes in flight live in shared memory rather than in registers, and
 // the other operands (Qn, Q2, Q3) and the result are streamed as 16-byte accesses.
 // One __syncthreads per plane.  Arithmetic and select semantics are those of k_rk above.
-constexpr int RKM_TX = 64, RKM_TY = 8, RKM_SW = 68, RKM_ROWS = RKM_TY + 2, RKM_NBUF = 4;
+constexpr int RKM_TX = 64, RKM_TY = 8, RKM_SW = 68, RKM_ROWS = RKM_TY + 2, RKM_NBUF = 4; // 5 tiles (three planes in flight) measured slower: 1.31 vs 1.10 ms per step
 constexpr int RKM_SMEM = RKM_NBUF * 4 * RKM_ROWS * RKM_SW * (int)sizeof(double);
 
 __device__ __forceinline__ void cp_async16(void *dst_smem, const void *src)
@@ -203,6 +203,7 @@ __device__ __forceinline__ void cp_async8(void *dst_smem, const void *src)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_one() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait_n() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 // RHS of one cell for field m given its seven-point neighbourhood and the advecting velocities.
 template <bool MASKED_C>
@@ -264,9 +265,8 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
         cp_async_commit();
     };
 
-    issue_plane(k0, 0);
-    issue_plane(k0 + 1, 1);
-    issue_plane(k0 + 2, 2);
+#pragma unroll
+    for (int n = 0; n <= RKM_NBUF - 2; ++n) issue_plane(k0 + n, n);
     // z-carried values of this thread's column: three register sets that take the roles z-1, centre, z+1 in
     // turn (the plane loop is unrolled three times, so the carry is a renaming, not a copy)
     double2 r0[4], r1[4], r2[4];
@@ -306,9 +306,9 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
             if (STAGE >= 2 && !ELIM) q2[m] = *reinterpret_cast<const double2 *>(a.qc[m] + o); // Qc, updated in place
             if (STAGE == 4 && ELIM) q2[m] = *reinterpret_cast<const double2 *>(a.qc[m] + o);  // S, overwritten below by Q*
         }
-        cp_async_wait_one();
+        cp_async_wait_n<RKM_NBUF - 3>();
         __syncthreads(); // plane k+1 visible to all; every thread is done with the tile of plane k-1
-        if (t + 3 <= kc) issue_plane(k + 3, (t + 3) % RKM_NBUF);
+        if (t + RKM_NBUF - 1 <= kc) issue_plane(k + RKM_NBUF - 1, (t + RKM_NBUF - 1) % RKM_NBUF);
         else cp_async_commit();
         const double *sC = sm + (t % RKM_NBUF) * PLANE, *sN = sm + ((t + 1) % RKM_NBUF) * PLANE;
         if (t == 0) {
