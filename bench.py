@@ -98,12 +98,19 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
 
+    def wait_ready(self, timeout=5.0):
+        """Block until nvidia-smi has delivered its first row, so that a short timed region is still sampled."""
+        t_end = time.time() + timeout
+        while self.proc is not None and not self.rows and time.time() < t_end:
+            time.sleep(0.02)
+
     def stop(self, t0, t1):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.15)
         self.proc.terminate()
-        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.2] or [r for (_, r) in self.rows]
+        inside = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.2]
+        rows = inside or [r for (_, r) in self.rows]
         sm, mx, reasons = [], [], set()
         for r in rows:
             try:
@@ -113,8 +120,12 @@ class ClockSampler:
             for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[2:6]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
-        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+        out = {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+               "reasons": sorted(reasons), "samples": len(sm), "samples_in_timed_region": len(inside)}
+        if not inside:
+            # nothing was sampled while the timed steps ran: what is reported is NOT the clock under load
+            out["note"] = "no nvidia-smi sample fell inside the timed region; values are from outside it (use more --steps)"
+        return out
 
 
 def job_value(ms_local, n_cells, steps, world, device):
@@ -212,6 +223,9 @@ def run_ours(args):
     s.step(W)
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.wait_ready()
+    barrier()
     l0 = s.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0 = time.time()
