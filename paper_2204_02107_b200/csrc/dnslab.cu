@@ -228,7 +228,9 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
         a.rev = (h->st_rev >> (STAGE - 1)) & 1;
         const dim3 blk(32, dnsst::RKM_TY, 1);
         const dim3 grd(h->P.nx / dnsst::RKM_TX, h->P.ny / dnsst::RKM_TY, h->P.nz / h->rk_kc);
-        const size_t smem = dnsst::RKM_SMEM;
+        // experiment hook: DNSLAB_RK_SMEM_PAD adds unused shared memory, e.g. to leave one block per SM instead of two
+        static const size_t pad = getenv("DNSLAB_RK_SMEM_PAD") ? (size_t)atol(getenv("DNSLAB_RK_SMEM_PAD")) : 0;
+        const size_t smem = dnsst::RKM_SMEM + pad;
 #define DNS_LAUNCH_MARCH(M, S)                                                                                   \
     do {                                                                                                         \
         auto kern = dnsst::k_rk_march<STAGE, ELIM, M, S>;                                                        \
