@@ -414,6 +414,128 @@ def test_source_table_eq5():
     assert half.max() <= 1.0
 
 
+# ---------------------------------------------------------------- source relaxation term of eqs. 2-3 (P18)
+# S (phi_set - phi)/tau_f, PAPER.md:49-52 (eqs. 2-3); readings R8-R10.  Closed forms only: nothing
+# below calls the oracle to make its own expectation.
+def _src(lo, size, u_set=(0.0, 0.0, 0.0), c_set=0.0, tau_f=1.0, comps=0xF, B=(0.0, 0.0, 0.0)):
+    return dict(lo=lo, size=size, B=B, u_set=u_set, c_set=c_set, tau_f=tau_f, comps=comps)
+
+
+def _box_indicator(shape, lo, size):
+    """1 inside the index box lo..lo+size-1 (x,y,z order, wrapping), written from index arithmetic."""
+    nz, ny, nx = shape
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    return (((i - lo[0]) % nx < size[0]) & ((j - lo[1]) % ny < size[1]) & ((k - lo[2]) % nz < size[2])).astype(float)
+
+
+@pytest.mark.parametrize("comps", range(16))
+def test_P18_source_zero_field_binary_box_every_component_mask(comps):
+    """Zero fields, binary box (B <= 0): F_phi = phi_set/tau_f inside the box for the enabled components (bit m of
+    `comps` <-> m-th of u,v,w,c), exactly 0 everywhere else and for the disabled ones."""
+    shape, tau = (8, 12, 16), 0.37
+    sets = (0.9, -1.7, 2.3, 0.6)
+    lo, size = (13, 3, 6), (6, 4, 5)          # wraps through the x seam and the z seam
+    o = mk(shape, (0.5, 0.25, 0.2), nu=0.3, alpha_c=0.2, sources=[_src(lo, size, sets[:3], sets[3], tau, comps)])
+    z = np.zeros(shape)
+    F = o.rhs(z, z, z, z)
+    inside = _box_indicator(shape, lo, size)
+    assert inside.sum() == 6 * 4 * 5
+    for m in range(4):
+        expect = inside * (sets[m] / tau) if comps & (1 << m) else z
+        assert np.array_equal(F[m], expect), (comps, m)
+
+
+def test_P18_source_relaxation_exact_rk4_decay_towards_the_set_value():
+    """S == 1 over the whole periodic box, uniform fields, no mask: convection, diffusion and the divergence vanish
+    identically, so each component obeys d(phi)/dt = (phi_set - phi)/tau_f and RK4 gives
+    phi_n = phi_set + (phi_0 - phi_set) G(-dt/tau_f)^n with the polynomial G of P7/P8."""
+    shape, dt, tau, n = (8, 8, 16), 0.05, 0.13, 5
+    sets, init = (0.8, -0.3, 0.45, 2.0), (0.1, 0.2, -0.15, 0.5)
+    o = mk(shape, (0.1, 0.2, 0.15), nu=0.0, alpha_c=0.0, dt=dt,
+           sources=[_src((3, 1, 5), (16, 8, 8), sets[:3], sets[3], tau)])
+    one = np.ones(shape)
+    o.set_fields(*(v * one for v in init))
+    o.step(n)
+    f = o.fields()
+    g = _G(-dt / tau).real ** n
+    for m, key in enumerate("uvwc"):
+        expect = sets[m] + (init[m] - sets[m]) * g
+        assert np.abs(f[key] - expect).max() < 1e-14, key
+    assert np.abs(f["p"]).max() < 1e-14
+    # a different tau_f per source, one source per component: each decays at its own rate
+    taus = (0.07, 0.11, 0.2, 0.31)
+    o = mk(shape, (0.1, 0.2, 0.15), dt=dt, sources=[_src((0, 0, 0), (16, 8, 8), sets[:3], sets[3], taus[m], 1 << m)
+                                                    for m in range(4)])
+    o.set_fields(*(v * one for v in init))
+    o.step(n)
+    f = o.fields()
+    for m, key in enumerate("uvwc"):
+        expect = sets[m] + (init[m] - sets[m]) * _G(-dt / taus[m]).real ** n
+        assert np.abs(f[key] - expect).max() < 1e-14, key
+
+
+def test_P18_overlapping_sources_add():
+    """Two boxes that overlap: F = sum_s S_s (set_s - phi)/tau_s (reading R8), here with a uniform non-zero field."""
+    shape = (8, 8, 16)
+    a = _src((2, 1, 1), (8, 5, 4), (1.0, 0.5, -0.25), 0.7, 0.2)
+    b = _src((6, 3, 2), (6, 4, 5), (-2.0, 0.125, 0.75), 0.1, 0.5, comps=0b1011)   # b does not force w
+    o = mk(shape, (1.0, 1.0, 1.0), sources=[a, b])
+    phi = (0.3, -0.2, 0.1, 0.4)
+    one = np.ones(shape)
+    F = o.rhs(*(v * one for v in phi))
+    Ia, Ib = _box_indicator(shape, a["lo"], a["size"]), _box_indicator(shape, b["lo"], b["size"])
+    assert (Ia * Ib).sum() == 4 * 3 * 3                     # they do overlap
+    seta, setb = a["u_set"] + (a["c_set"],), b["u_set"] + (b["c_set"],)
+    for m in range(4):
+        eb = Ib * (setb[m] - phi[m]) / b["tau_f"] if b["comps"] & (1 << m) else 0.0
+        expect = Ia * (seta[m] - phi[m]) / a["tau_f"] + eb
+        assert np.abs(F[m] - expect).max() < 1e-15, m
+
+
+def test_P18_smooth_source_enters_to_the_first_power():
+    """B > 0 (eq. 5): F = S_x S_y S_z phi_set/tau_f with each factor the tanh window written out here
+    -- the first power of S, and the product of the three one-dimensional factors."""
+    shape, d = (16, 16, 32), (0.25, 0.5, 0.125)
+    lo, size, B = (10, 4, 5), (9, 5, 7), (4.0, 2.5, 3.0)
+    tau, cset = 0.4, 1.5
+
+    def window(n, h, l, s, b):
+        xc, w2 = (l + 0.5 * (s - 1)) * h, 0.5 * s * h
+        r = np.abs(np.arange(n) * h - xc)
+        r = np.minimum(r, n * h - r)                       # minimum image
+        with np.errstate(divide="ignore"):
+            return 0.5 * (1.0 - np.tanh(b * (r / w2 - w2 / r)))
+
+    sx, sy, sz = (window(shape[2 - a], d[a], lo[a], size[a], B[a]) for a in range(3))
+    S = sz[:, None, None] * sy[None, :, None] * sx[None, None, :]
+    assert S.max() == 1.0 and ((S > 0.1) & (S < 0.9)).sum() > 50          # really smooth: S and S^2 differ
+    o = mk(shape, d, sources=[_src(lo, size, (0.0, 0.0, -1.0), cset, tau, comps=0b1100, B=B)])
+    z = np.zeros(shape)
+    F = o.rhs(z, z, z, z)
+    assert np.abs(F[3] - S * cset / tau).max() < 1e-15 and np.abs(F[2] + S / tau).max() < 1e-15
+    assert not F[0].any() and not F[1].any()
+    assert np.abs(F[3] - S * S * cset / tau).max() > 0.1              # what a squared window would give
+
+
+def test_P18_set_fields_selects_plus_zero_in_solid_cells():
+    """PAPER.md:58 as a select (reading R7): whatever the caller passes in solid cells -- here large values, negative
+    values and a NaN -- is stored as +0.0; fluid cells and the whole of p are stored untouched."""
+    r = rng(21)
+    shape = (6, 8, 10)
+    mask = (r.random(shape) < 0.6).astype(np.uint8)
+    o = mk(shape, mask=mask)
+    fld = [r.standard_normal(shape) * 1e3 - 5.0 for _ in range(5)]
+    solid = mask == 0
+    fld[0][solid] = -7.0
+    fld[3][tuple(np.argwhere(solid)[0])] = np.nan
+    o.set_fields(*fld[:4], p=fld[4])
+    f = o.fields()
+    for m, key in enumerate("uvwc"):
+        assert np.all(f[key][solid] == 0.0) and not np.any(np.signbit(f[key][solid])), key
+        assert np.array_equal(f[key][~solid], fld[m][~solid]), key
+    assert np.array_equal(f["p"], fld[4])
+
+
 # ---------------------------------------------------------------- symmetries (P14)
 def _run_case(case, steps, n_piter=None):
     o = mk(case["shape"], case["d"], nu=case["nu"], alpha_c=case["alpha_c"], dt=case["dt"], mask=case["mask"],
