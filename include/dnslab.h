@@ -56,12 +56,10 @@ typedef struct {
     double body[3];        /* body force b (eq. 2)                                      */
     int32_t n_piter;       /* eq. 9 iterations >= 1; the paper hard-codes 4           */
     uint32_t flags;        /* bit0: eq. 6 filter on u,v,w,c at the end of every step (PAPER.md:84-88,
-                              central 7-point stencil, gamma = Delta^6/pi^6); bit1: project every RK stage;
-                              bit2: evaluate eq. 9's right-hand side densely inside the forward x pass
-                              instead of at the listed near-solid cells (same result; the library does
-                              this by itself when more than half of the cells are near-solid);
-                              bit3: two RK stages per launch (k_rk_pair: the intermediate stage field
-                              stays in shared memory; same result up to rounding; experimental)       */
+                              central 7-point stencil, gamma = Delta^6/pi^6 as printed: a one-axis Nyquist
+                              mode is damped by 0.933 per step, not zeroed -- DESIGN.md reading R23);
+                              bit1: project every RK stage (what PAPER.md:43 says the authors dropped for
+                              speed).  Any other bit set: DNSLAB_EINVAL                                  */
 } dnslab_params_t;
 
 /* One inflow/outflow forcing region S(x,y,z) of eqs. 2-3. */
@@ -80,7 +78,8 @@ size_t dnslab_workspace_bytes(const dnslab_params_t *params);
 
 /*
  * Create a solver.  mask: nx*ny*nz bytes (host or device pointer; NULL = all fluid), copied.
- * src: nsrc (<= DNSLAB_MAX_SOURCES) host structs, copied.  workspace: DEVICE memory, caller-owned,
+ * src: nsrc (<= DNSLAB_MAX_SOURCES) host structs, copied; each needs tau_f > 0 and 1 <= size[a] <= N_a
+ * (else DNSLAB_EINVAL).  workspace: DEVICE memory, caller-owned,
  * at least dnslab_workspace_bytes() bytes, 256-byte aligned; it must outlive the handle.
  * cuda_stream: a cudaStream_t (NULL = default stream); every later call runs on it.
  * All fields start at 0 (p = 0 is the first warm start).  Synchronous.

@@ -101,14 +101,19 @@ def workspace_bytes(params):
     return int(lib().dnslab_workspace_bytes(C.byref(params)))
 
 
-def _addr(x):
-    """Address of a torch tensor (device or host), a numpy array, or None."""
+def _addr(x, dtype="float64"):
+    """Address of a contiguous torch tensor (device or host) or numpy array of the given dtype, or None.
+    The library reads raw bytes: a wrong dtype would be an out-of-bounds read, so it is refused here."""
     if x is None:
         return None
+    if str(x.dtype).split(".")[-1] != dtype:
+        raise DnslabError(f"expected a {dtype} buffer, got {x.dtype}")
     if hasattr(x, "data_ptr"):
-        assert x.is_contiguous()
+        if not x.is_contiguous():
+            raise DnslabError("buffer must be contiguous")
         return x.data_ptr()
-    assert x.flags["C_CONTIGUOUS"]
+    if not x.flags["C_CONTIGUOUS"]:
+        raise DnslabError("buffer must be contiguous")
     return x.ctypes.data
 
 
@@ -142,7 +147,7 @@ class Solver:
             import numpy as np
             mask = np.ascontiguousarray(mask, dtype=np.uint8)
         self._mask = mask
-        _check(lib().dnslab_create(C.byref(self.params), _addr(mask), self._src, len(sources), self._ws_ptr,
+        _check(lib().dnslab_create(C.byref(self.params), _addr(mask, "uint8"), self._src, len(sources), self._ws_ptr,
                                    self.stream.cuda_stream, C.byref(self._h)), "dnslab_create")
 
     # -- C ABI calls ---------------------------------------------------------------------

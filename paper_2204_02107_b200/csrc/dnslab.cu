@@ -20,6 +20,11 @@ using dnsfft::c2;
 namespace {
 
 constexpr size_t ALIGN = 256;
+// Tile traversal direction, one bit per kernel (set: walk from the far end, i.e. start on what the kernel before left
+// in the 126 MB L2).  Measured sweeps on 512x256x128: the y passes gain from walking against the x passes
+// (41.7 instead of 45 us each); of the stencil kernels only the divergence gains (83 instead of 88 us).
+constexpr int FFT_REV = 10; // bits: x fwd, y fwd, z, y inv, x inv
+constexpr int ST_REV = 16;  // bits: RK stages 1-4, divergence, projection
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 inline bool pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 
@@ -30,7 +35,7 @@ bool valid_params(const dnslab_params_t *P)
     if (P->nx < 8 || P->nx > 2048 || P->ny < 8 || P->ny > 1024 || P->nz < 8 || P->nz > 1024) return false;
     if (!(P->dx > 0) || !(P->dy > 0) || !(P->dz > 0) || !(P->dt > 0)) return false;
     if (!(P->nu >= 0) || !(P->alpha_c >= 0) || P->n_piter < 1) return false;
-    if (P->flags & ~15u) return false;
+    if (P->flags & ~3u) return false;
     return true;
 }
 
@@ -112,14 +117,11 @@ struct dnslab {
     int64_t launches;
     dim3 rk_block;
     int nsm;   // SM count of the device
-    int z_oneshot; // fused z pass: one tile per block instead of the persistent kernel (env DNSLAB_Z_ONESHOT)
-    int st_rev;  // bit per stencil kernel of a step (RK stages 1-4, divergence, projection): same idea
-    int fft_rev; // bit per pass of a solve (x fwd, y fwd, z, y inv, x inv): walk its tiles from the far end
+    bool prepare; // set while dnslab_create walks the launchers once: they configure their kernel and do not launch
+    unsigned zgrid; // grid of the persistent fused z pass (occupancy query done once, at create)
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
     long long np;      // NEXT-4: attached particles (0: none); state is the caller's device array
     double *pstate, prho_f, pgrav[3];
-    int pair_mode; // 0: stages 1+2 and 3+4 fused; 1: only stages 1+2 fused (env DNSLAB_PAIR_MODE)
-    int pair_kc; // > 0: two-stage kernel (k_rk_pair) with this many planes per block; 0: one launch per stage
     // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
     bool prof_on;
     std::vector<ProfRec> *prof;
@@ -190,7 +192,7 @@ dim3 tile_block(const dnslab *h)
 
 // ---- RK stage ---------------------------------------------------------------------------
 // qs: stage field (stencil input); qo: next stage field; elim: Qc eliminated
-template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, double *const *qo, double *const *q2, double *const *q3)
+template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, double *const *qo, double *const *q2)
 {
     static const double ca[4] = {0.5, 0.5, 1.0, 0.0};
     static const double cb[4] = {1.0 / 6.0, 1.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0};
@@ -200,7 +202,6 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
         a.qs[m] = qs[m];
         a.qn[m] = h->Q[m];
         a.qc[m] = ELIM ? (q2 ? q2[m] : nullptr) : h->Qc[m];
-        a.q3[m] = q3 ? q3[m] : nullptr;
         a.qo[m] = qo ? qo[m] : nullptr;
         a.qco[m] = ELIM ? (q2 ? q2[m] : nullptr) : h->Qc[m];
     }
@@ -221,22 +222,19 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
     a.stab = h->stab;
     for (int s = 0; s < h->nsrc; ++s) a.src[s] = h->src[s];
     const bool masked = h->face != nullptr, sources = h->nsrc > 0;
-    ProfScope ps(h, DNSLAB_K_RK);
     if (h->rk_kc > 0) {
         // z-marching kernel: 64 x 8 columns, kc planes per block
         a.kc = h->rk_kc;
-        a.rev = (h->st_rev >> (STAGE - 1)) & 1;
+        a.rev = (ST_REV >> (STAGE - 1)) & 1;
         const dim3 blk(32, dnsst::RKM_TY, 1);
         const dim3 grd(h->P.nx / dnsst::RKM_TX, h->P.ny / dnsst::RKM_TY, h->P.nz / h->rk_kc);
-        // experiment hook: DNSLAB_RK_SMEM_PAD adds unused shared memory, e.g. to leave one block per SM instead of two
-        static const size_t pad = getenv("DNSLAB_RK_SMEM_PAD") ? (size_t)atol(getenv("DNSLAB_RK_SMEM_PAD")) : 0;
-        const size_t smem = dnsst::RKM_SMEM + pad;
-#define DNS_LAUNCH_MARCH(M, S)                                                                                   \
-    do {                                                                                                         \
-        auto kern = dnsst::k_rk_march<STAGE, ELIM, M, S>;                                                        \
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)   \
-            return DNSLAB_ECUDA;                                                                                 \
-        kern<<<grd, blk, smem, h->stream>>>(a);                                                                  \
+        const size_t smem = dnsst::RKM_SMEM;
+#define DNS_LAUNCH_MARCH(M, S)                                                                                          \
+    do {                                                                                                                \
+        auto kern = dnsst::k_rk_march<STAGE, ELIM, M, S>;                                                               \
+        if (h->prepare) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess ? DNSLAB_OK : DNSLAB_ECUDA; \
+        ProfScope ps(h, DNSLAB_K_RK);                                                                                   \
+        kern<<<grd, blk, smem, h->stream>>>(a);                                                                         \
     } while (0)
         if (masked && sources) DNS_LAUNCH_MARCH(true, true);
         else if (masked) DNS_LAUNCH_MARCH(true, false);
@@ -245,60 +243,14 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
 #undef DNS_LAUNCH_MARCH
         return check_launch(h);
     }
+    if (h->prepare) return DNSLAB_OK;
+    ProfScope ps(h, DNSLAB_K_RK);
     const dim3 blk = h->rk_block;
     const dim3 grd(h->P.nx / blk.x, h->P.ny / blk.y, h->P.nz / blk.z);
     if (masked && sources) dnsst::k_rk<STAGE, ELIM, true, true><<<grd, blk, 0, h->stream>>>(a);
     else if (masked) dnsst::k_rk<STAGE, ELIM, true, false><<<grd, blk, 0, h->stream>>>(a);
     else if (sources) dnsst::k_rk<STAGE, ELIM, false, true><<<grd, blk, 0, h->stream>>>(a);
     else dnsst::k_rk<STAGE, ELIM, false, false><<<grd, blk, 0, h->stream>>>(a);
-    return check_launch(h);
-}
-
-// Two stages per launch (k_rk_pair): PAIR 0 = stages 1+2 (Qn -> Q2, Q3), PAIR 1 = stages 3+4 (Q3, Qn, Q2 -> Q* in place of Q2)
-template <int PAIR> int launch_rk_pair(dnslab *h, double *const *qs, double *const *q2, double *const *q3)
-{
-    dnsst::RKArgs a;
-    std::memset(&a, 0, sizeof(a));
-    for (int m = 0; m < 4; ++m) {
-        a.qs[m] = qs[m];
-        a.qn[m] = h->Q[m];
-        a.qc[m] = q2[m];
-        a.qo[m] = q2[m];
-        a.qco[m] = PAIR == 0 ? q3[m] : q2[m];
-    }
-    a.face = h->face;
-    a.nx = h->P.nx; a.ny = h->P.ny; a.nz = h->P.nz;
-    a.r2x = 1.0 / (2.0 * h->P.dx); a.r2y = 1.0 / (2.0 * h->P.dy); a.r2z = 1.0 / (2.0 * h->P.dz);
-    a.rxx = 1.0 / (h->P.dx * h->P.dx); a.ryy = 1.0 / (h->P.dy * h->P.dy); a.rzz = 1.0 / (h->P.dz * h->P.dz);
-    a.nu = h->P.nu; a.ac = h->P.alpha_c;
-    for (int m = 0; m < 3; ++m) a.body[m] = h->P.body[m];
-    a.kf.hx = -0.5 * a.r2x; a.kf.hy = -0.5 * a.r2y; a.kf.hz = -0.5 * a.r2z;
-    a.kf.dvx = a.nu * a.rxx; a.kf.dvy = a.nu * a.ryy; a.kf.dvz = a.nu * a.rzz;
-    a.kf.dcx = a.ac * a.rxx; a.kf.dcy = a.ac * a.ryy; a.kf.dcz = a.ac * a.rzz;
-    a.kf.dv0 = -2.0 * (a.kf.dvx + a.kf.dvy + a.kf.dvz);
-    a.kf.dc0 = -2.0 * (a.kf.dcx + a.kf.dcy + a.kf.dcz);
-    a.ca = (PAIR == 0 ? 0.5 : 1.0) * h->P.dt;
-    a.cb = (PAIR == 0 ? 0.5 : 1.0 / 6.0) * h->P.dt;
-    a.nsrc = h->nsrc;
-    a.stab = h->stab;
-    for (int s = 0; s < h->nsrc; ++s) a.src[s] = h->src[s];
-    a.kc = h->pair_kc;
-    const bool masked = h->face != nullptr, sources = h->nsrc > 0;
-    const dim3 grd(h->P.nx / dnsst::P2_TX, h->P.ny / dnsst::P2_TY, h->P.nz / h->pair_kc);
-    const size_t smem = PAIR == 0 ? dnsst::P2_SMEM0 : dnsst::P2_SMEM1;
-    ProfScope ps(h, DNSLAB_K_RK);
-#define DNS_LAUNCH_PAIR(M, S)                                                                                    \
-    do {                                                                                                         \
-        auto kern = dnsst::k_rk_pair<PAIR, M, S>;                                                                \
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)   \
-            return DNSLAB_ECUDA;                                                                                 \
-        kern<<<grd, dnsst::P2_NT, smem, h->stream>>>(a);                                                         \
-    } while (0)
-    if (masked && sources) DNS_LAUNCH_PAIR(true, true);
-    else if (masked) DNS_LAUNCH_PAIR(true, false);
-    else if (sources) DNS_LAUNCH_PAIR(false, true);
-    else DNS_LAUNCH_PAIR(false, false);
-#undef DNS_LAUNCH_PAIR
     return check_launch(h);
 }
 
@@ -328,9 +280,10 @@ template <int L, int DIR, bool PRO> int launch_fft_x_L(dnslab *h, const c2 *in, 
     const size_t nlines = (size_t)h->P.ny * h->P.nz;
     size_t nl = 128 / T;
     if (nl > nlines) nl = nlines;
-    const size_t smem = nl * (L + L / 8) * sizeof(c2);
+    const size_t smem = nl * (L + L / 8) * sizeof(c2); // <= 18 KB: no opt-in needed
+    if (h->prepare) return DNSLAB_OK;
     ProfScope ps(h, DNSLAB_K_FFT_X);
-    dnsfft::k_fft_x<L, DIR, PRO><<<(unsigned)(nlines / nl), (unsigned)(nl * T), smem, h->stream>>>(in, out, h->tw[0], (int)nl, (h->fft_rev >> (DIR < 0 ? 0 : 4)) & 1, ra);
+    dnsfft::k_fft_x<L, DIR, PRO><<<(unsigned)(nlines / nl), (unsigned)(nl * T), smem, h->stream>>>(in, out, h->tw[0], (int)nl, (FFT_REV >> (DIR < 0 ? 0 : 4)) & 1, ra);
     return check_launch(h);
 }
 
@@ -360,9 +313,12 @@ template <int L, int XT, int DIR> int launch_fft_col_LX(dnslab *h, c2 *data, int
     const int nother = axis == 1 ? h->P.nz : h->P.ny;
     const size_t smem = (size_t)XT * L * sizeof(c2);
     auto kern = dnsfft::k_fft_col<L, XT, DIR>;
-    if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (h->prepare) {
+        if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        return DNSLAB_OK;
+    }
     ProfScope ps(h, DNSLAB_K_FFT_Y);
-    kern<<<(unsigned)((mx / XT) * nother), XT * T, smem, h->stream>>>(data, h->tw[axis], mx, stride, other_stride, (h->fft_rev >> (DIR < 0 ? 1 : 3)) & 1);
+    kern<<<(unsigned)((mx / XT) * nother), XT * T, smem, h->stream>>>(data, h->tw[axis], mx, stride, other_stride, (FFT_REV >> (DIR < 0 ? 1 : 3)) & 1);
     return check_launch(h);
 }
 
@@ -395,21 +351,11 @@ template <int L, int XT> int launch_fft_z_solve_LX(dnslab *h, c2 *data)
     const int mx = h->P.nx / 2;
     const size_t smem = 2 * (size_t)XT * L * sizeof(c2);
     const size_t ntiles = (size_t)(mx / XT) * h->P.ny;
-    if (h->z_oneshot) {
-        const size_t smem1 = (size_t)XT * L * sizeof(c2);
-        auto kern1 = dnsfft::k_fft_z_solve1<L, XT>;
-        if (smem1 > 48 * 1024) CK(cudaFuncSetAttribute(kern1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
-        ProfScope ps(h, DNSLAB_K_FFT_Z);
-        kern1<<<(unsigned)ntiles, XT * T, smem1, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2],
-                                                              2.0 / (double)h->n, (h->fft_rev >> 2) & 1);
-        return check_launch(h);
-    }
     auto kern = dnsfft::k_fft_z_solve<L, XT>;
-    unsigned grid = 0;
-    if (int rc = persistent_grid(h, kern, NT, smem, ntiles, &grid)) return rc;
+    if (h->prepare) return persistent_grid(h, kern, NT, smem, ntiles, &h->zgrid);
     ProfScope ps(h, DNSLAB_K_FFT_Z);
     const double inv_n = 2.0 / (double)h->n; // the packed transform has n/2 complex points
-    kern<<<grid, XT * T, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], inv_n, (int)ntiles, (h->fft_rev >> 2) & 1);
+    kern<<<h->zgrid, XT * T, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], inv_n, (int)ntiles, (FFT_REV >> 2) & 1);
     return check_launch(h);
 }
 
@@ -461,7 +407,7 @@ int launch_div(dnslab *h, double *const *q)
     if (h->P.nx >= 64 && h->P.ny >= 8) {
         const dim3 blk2(32, 8, 1), grd2(h->P.nx / 64, h->P.ny / 8, h->P.nz);
         dnsst::k_div2<<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], h->d, h->P.nx, h->P.ny, h->P.nz, 1.0 / (2.0 * h->P.dx),
-                                                    1.0 / (2.0 * h->P.dy), 1.0 / (2.0 * h->P.dz), (h->st_rev >> 4) & 1);
+                                                    1.0 / (2.0 * h->P.dy), 1.0 / (2.0 * h->P.dz), (ST_REV >> 4) & 1);
         return check_launch(h);
     }
     const dim3 blk = tile_block(h);
@@ -479,8 +425,8 @@ int launch_project(dnslab *h, double *const *q, const double *p)
     ProfScope ps(h, DNSLAB_K_PROJECT);
     if (h->P.nx >= 64 && h->P.ny >= 8) {
         const dim3 blk2(32, 8, 1), grd2(h->P.nx / 64, h->P.ny / 8, h->P.nz);
-        if (h->face) dnsst::k_project2<true><<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], p, h->face, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z, (h->st_rev >> 5) & 1);
-        else dnsst::k_project2<false><<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], p, nullptr, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z, (h->st_rev >> 5) & 1);
+        if (h->face) dnsst::k_project2<true><<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], p, h->face, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z, (ST_REV >> 5) & 1);
+        else dnsst::k_project2<false><<<grd2, blk2, 0, h->stream>>>(q[0], q[1], q[2], p, nullptr, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z, (ST_REV >> 5) & 1);
         return check_launch(h);
     }
     if (h->face) dnsst::k_project<true><<<grd, blk, 0, h->stream>>>(q[0], q[1], q[2], p, h->face, h->P.nx, h->P.ny, h->P.nz, r2x, r2y, r2z);
@@ -514,8 +460,13 @@ int launch_filter(dnslab *h, double *const *in, double *const *out)
     a.nx = h->P.nx; a.ny = h->P.ny; a.nz = h->P.nz;
     const double pi = 3.14159265358979323846;
     a.g = 1.0 / (pi * pi * pi * pi * pi * pi);
+    if (h->prepare) { // the only kernels here that need the shared-memory opt-in
+        CK(cudaFuncSetAttribute(dnsst::k_filter_march<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dnsst::FM_SMEM));
+        CK(cudaFuncSetAttribute(dnsst::k_filter_march<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dnsst::FM_SMEM));
+        return DNSLAB_OK;
+    }
     ProfScope ps(h, DNSLAB_K_FILTER);
-    if (h->P.nx >= dnsst::FM_TX && h->P.ny >= dnsst::FM_TY && !getenv("DNSLAB_FILTER_SIMPLE")) {
+    if (h->P.nx >= dnsst::FM_TX && h->P.ny >= dnsst::FM_TY) {
         // z-marching kernel: 64 x 8 columns of one field; >= 4 waves of 4 blocks per SM, at least 8 planes per block
         const long tiles = 4L * (h->P.nx / dnsst::FM_TX) * (h->P.ny / dnsst::FM_TY);
         int kc = h->P.nz;
@@ -524,13 +475,8 @@ int launch_filter(dnslab *h, double *const *in, double *const *out)
         const dim3 blk(32, dnsst::FM_TY, 1);
         const dim3 grd(h->P.nx / dnsst::FM_TX, h->P.ny / dnsst::FM_TY, 4 * (h->P.nz / kc));
         const size_t smem = dnsst::FM_SMEM;
-        if (h->face) {
-            CK(cudaFuncSetAttribute(dnsst::k_filter_march<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            dnsst::k_filter_march<true><<<grd, blk, smem, h->stream>>>(a);
-        } else {
-            CK(cudaFuncSetAttribute(dnsst::k_filter_march<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            dnsst::k_filter_march<false><<<grd, blk, smem, h->stream>>>(a);
-        }
+        if (h->face) dnsst::k_filter_march<true><<<grd, blk, smem, h->stream>>>(a);
+        else dnsst::k_filter_march<false><<<grd, blk, smem, h->stream>>>(a);
         return check_launch(h);
     }
     const dim3 blk(h->P.nx < 32 ? h->P.nx : 32, h->P.ny < 8 ? h->P.ny : 8, 1);
@@ -573,6 +519,26 @@ int pressure_stage(dnslab *h, double *const *q, double *p)
     return launch_project(h, q, p);
 }
 
+// called once from dnslab_create with h->prepare set: nothing is launched
+int prepare_kernels(dnslab *h)
+{
+    int rc;
+    if (h->P.flags & 2u) {
+        if ((rc = launch_rk<1, false>(h, h->Q, h->A, nullptr))) return rc;
+        if ((rc = launch_rk<2, false>(h, h->A, h->Bf, nullptr))) return rc;
+        if ((rc = launch_rk<3, false>(h, h->Bf, h->A, nullptr))) return rc;
+        if ((rc = launch_rk<4, false>(h, h->A, nullptr, nullptr))) return rc;
+    } else {
+        if ((rc = launch_rk<1, true>(h, h->Q, h->A, nullptr))) return rc;
+        if ((rc = launch_rk<2, true>(h, h->A, h->Bf, h->Qc))) return rc;
+        if ((rc = launch_rk<3, true>(h, h->Bf, h->A, nullptr))) return rc;
+        if ((rc = launch_rk<4, true>(h, h->A, nullptr, h->Qc))) return rc;
+    }
+    if ((rc = poisson_solve(h, h->d, h->p, h->p, true))) return rc;
+    if ((h->P.flags & 1u) && (rc = launch_filter(h, h->Qc, h->A))) return rc;
+    return DNSLAB_OK;
+}
+
 } // namespace
 
 extern "C" {
@@ -600,8 +566,12 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
 {
     if (!valid_params(params) || !workspace || !out || nsrc < 0 || nsrc > DNSLAB_MAX_SOURCES || (nsrc > 0 && !src)) return DNSLAB_EINVAL;
     if ((uintptr_t)workspace % ALIGN) return DNSLAB_EINVAL;
-    for (int s = 0; s < nsrc; ++s)
+    for (int s = 0; s < nsrc; ++s) {
         if (!(src[s].tau_f > 0)) return DNSLAB_EINVAL;
+        const int nn[3] = {params->nx, params->ny, params->nz};
+        for (int a = 0; a < 3; ++a)
+            if (src[s].size[a] < 1 || src[s].size[a] > nn[a]) return DNSLAB_EINVAL; // eq. 5 divides by the half width
+    }
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return DNSLAB_EARCH;
@@ -614,11 +584,6 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
     h->n = (size_t)params->nx * params->ny * params->nz;
     h->stream = (cudaStream_t)cuda_stream;
     h->nsm = prop.multiProcessorCount;
-    h->fft_rev = 10; // y passes walk against the x passes: 41.7 instead of 45 us each (measured sweep over the 5-bit choices)
-    if (const char *v = getenv("DNSLAB_FFT_REV")) h->fft_rev = atoi(v);
-    h->z_oneshot = getenv("DNSLAB_Z_ONESHOT") ? atoi(getenv("DNSLAB_Z_ONESHOT")) : 0;
-    h->st_rev = 16; // only the divergence gains from it (83 instead of 88 us); the RK stages do not
-    if (const char *v = getenv("DNSLAB_ST_REV")) h->st_rev = atoi(v);
     h->ws = (char *)workspace;
     h->L = make_layout(params);
     const Layout &L = h->L;
@@ -636,35 +601,17 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
     {
         // 64 x 2 x 2 brick (256 threads); narrower in x on tiny grids
         unsigned bx = params->nx < 64 ? params->nx : 64, by = 2, bz = 2;
-        if (const char *v = getenv("DNSLAB_RK_BLOCK")) sscanf(v, "%u,%u,%u", &bx, &by, &bz);
         while (bx * by * bz < 256 && by < (unsigned)params->ny && by <= bz) by *= 2;
         while (bx * by * bz < 256 && bz < (unsigned)params->nz) bz *= 2;
         h->rk_block = dim3(bx, by, bz);
         // marching kernel for nx >= 64: enough blocks for >= 6 waves of 2 blocks per SM, at least 8 planes each
+        // (16 planes per block is the best of 8...128 on 512x256x128)
         h->rk_kc = 0;
-        if (params->nx >= dnsst::RKM_TX && !getenv("DNSLAB_RK_BRICK")) {
+        if (params->nx >= dnsst::RKM_TX) {
             const long tiles = (long)(params->nx / dnsst::RKM_TX) * (params->ny / dnsst::RKM_TY);
             int kc = params->nz;
             while (kc > 8 && tiles * (params->nz / kc) < 6L * 2 * prop.multiProcessorCount) kc /= 2;
-            if (const char *v = getenv("DNSLAB_RK_KC")) {
-                const int e = atoi(v);
-                if (e >= 1 && e <= params->nz && params->nz % e == 0) kc = e;
-            }
             h->rk_kc = kc;
-        }
-        // two stages per launch (flags bit 3) for nx >= 32, ny >= 16: one block per SM, >= 6 waves, at least 8 planes each
-        h->pair_kc = 0;
-        h->pair_mode = 0;
-        if (const char *v = getenv("DNSLAB_PAIR_MODE")) h->pair_mode = atoi(v);
-        if (params->nx >= dnsst::P2_TX && params->ny >= dnsst::P2_TY && ((params->flags & 8u) || getenv("DNSLAB_RK_PAIR"))) {
-            const long tiles = (long)(params->nx / dnsst::P2_TX) * (params->ny / dnsst::P2_TY);
-            int kc = params->nz;
-            while (kc > 8 && tiles * (params->nz / kc) < 6L * prop.multiProcessorCount) kc /= 2;
-            if (const char *v = getenv("DNSLAB_PAIR_KC")) {
-                const int e = atoi(v);
-                if (e >= 1 && e <= params->nz && params->nz % e == 0) kc = e;
-            }
-            h->pair_kc = kc;
         }
     }
 
@@ -691,7 +638,7 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
             if (!hm[o]) { any_solid = true; break; }
         if (any_solid) h->face = face;
         CKF(cudaMemsetAsync(h->W, 0, L.field_bytes, h->stream));
-        if (any_solid && !(params->flags & 4u)) {
+        if (any_solid) {
             // cells with at least one solid face neighbour, ascending index order
             const int nx = params->nx, ny = params->ny, nz = params->nz;
             std::vector<uint32_t> bl;
@@ -771,6 +718,12 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
     }
     CKF(cudaStreamSynchronize(h->stream));
 #undef CKF
+    // one dry walk over the launchers: each configures the kernel instantiation it will use (shared-memory
+    // opt-in, persistent grid size) and launches nothing, so that no launch path calls cudaFuncSetAttribute
+    h->prepare = true;
+    int prc = prepare_kernels(h);
+    h->prepare = false;
+    if (prc) return fail(prc);
     *out = h;
     return DNSLAB_OK;
 }
@@ -797,30 +750,18 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
     const size_t bytes = h->n * sizeof(double);
     int rc;
     for (int it = 0; it < nsteps; ++it) {
-        if (!stage_proj && h->pair_kc > 0 && h->pair_mode == 1) {
-            // stages 1+2 in one launch (Q2 stays on chip; Bf = Q3, Qc = S), then stages 3 and 4 as single launches
-            if ((rc = launch_rk_pair<0>(h, h->Q, h->Qc, h->Bf))) return rc;
-            if ((rc = launch_rk<3, true>(h, h->Bf, h->A, nullptr, nullptr))) return rc;
-            if ((rc = launch_rk<4, true>(h, h->A, nullptr, h->Qc, nullptr))) return rc;
-        } else if (!stage_proj && h->pair_kc > 0) {
-            // two launches: stages 1+2 (A = S, Bf = Q3), stages 3+4 (Q4 stays on chip, Q* overwrites A)
-            if ((rc = launch_rk_pair<0>(h, h->Q, h->A, h->Bf))) return rc;
-            if ((rc = launch_rk_pair<1>(h, h->Bf, h->A, h->Bf))) return rc;
-        } else if (!stage_proj) {
-            // Qc eliminated: A = Q2, Bf = Q3, Qc = S = Q2 - Qn + 2 Q3 (written by stage 2), A = Q4, Q* in place of S
-            if ((rc = launch_rk<1, true>(h, h->Q, h->A, nullptr, nullptr))) return rc;
-            if ((rc = launch_rk<2, true>(h, h->A, h->Bf, h->Qc, nullptr))) return rc;
-            if ((rc = launch_rk<3, true>(h, h->Bf, h->A, nullptr, nullptr))) return rc;
-            if ((rc = launch_rk<4, true>(h, h->A, nullptr, h->Qc, nullptr))) return rc;
-        }
         if (!stage_proj) {
-            // Q* is in A (two-stage kernels) or Qc (one kernel per stage); the other one is free for the filter
-            const bool inA = h->pair_kc > 0 && h->pair_mode != 1;
-            double **fin = inA ? h->A : h->Qc, **spare = inA ? h->Qc : h->A;
+            // Qc eliminated: A = Q2, Bf = Q3, Qc = S = Q2 - Qn + 2 Q3 (written by stage 2), A = Q4, Q* in place of S
+            if ((rc = launch_rk<1, true>(h, h->Q, h->A, nullptr))) return rc;
+            if ((rc = launch_rk<2, true>(h, h->A, h->Bf, h->Qc))) return rc;
+            if ((rc = launch_rk<3, true>(h, h->Bf, h->A, nullptr))) return rc;
+            if ((rc = launch_rk<4, true>(h, h->A, nullptr, h->Qc))) return rc;
+            // Q* is in Qc; A is free for the filter
+            double **fin = h->Qc;
             if ((rc = pressure_stage(h, fin, h->p))) return rc;
             if (filter) {
-                if ((rc = launch_filter(h, fin, spare))) return rc;
-                fin = spare;
+                if ((rc = launch_filter(h, fin, h->A))) return rc;
+                fin = h->A;
             }
             for (int m = 0; m < 4; ++m) {
                 double *t = h->Q[m];
@@ -831,16 +772,16 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
             continue;
         }
         // NEXT-2 variant: every stage field is projected, so the accumulate form is needed
-        if ((rc = launch_rk<1, false>(h, h->Q, h->A, nullptr, nullptr))) return rc;
+        if ((rc = launch_rk<1, false>(h, h->Q, h->A, nullptr))) return rc;
         CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
         if ((rc = pressure_stage(h, h->A, h->ps))) return rc;
-        if ((rc = launch_rk<2, false>(h, h->A, h->Bf, nullptr, nullptr))) return rc;
+        if ((rc = launch_rk<2, false>(h, h->A, h->Bf, nullptr))) return rc;
         CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
         if ((rc = pressure_stage(h, h->Bf, h->ps))) return rc;
-        if ((rc = launch_rk<3, false>(h, h->Bf, h->A, nullptr, nullptr))) return rc;
+        if ((rc = launch_rk<3, false>(h, h->Bf, h->A, nullptr))) return rc;
         CK(cudaMemcpyAsync(h->ps, h->p, bytes, cudaMemcpyDeviceToDevice, h->stream));
         if ((rc = pressure_stage(h, h->A, h->ps))) return rc;
-        if ((rc = launch_rk<4, false>(h, h->A, nullptr, nullptr, nullptr))) return rc;
+        if ((rc = launch_rk<4, false>(h, h->A, nullptr, nullptr))) return rc;
         if ((rc = pressure_stage(h, h->Qc, h->p))) return rc;
         double **fin = h->Qc;
         if (filter) {

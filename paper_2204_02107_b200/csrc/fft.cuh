@@ -390,42 +390,4 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 
     }
 }
 
-// One-shot variant of the fused z pass (one tile per block, elements loaded straight into registers), kept for
-// comparison with the persistent one (DNSLAB_Z_ONESHOT=1).
-template <int L, int XT>
-__global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 : XT *(L / ElemsPerThreadZ<L>::value))
-    k_fft_z_solve1(c2 *__restrict__ data, const c2 *__restrict__ tw, int mx, int ny, const double *__restrict__ ex,
-                   const double *__restrict__ ey, const double *__restrict__ ez, double inv_n, int rev)
-{
-    constexpr int E = ElemsPerThreadZ<L>::value;
-    constexpr int T = L / E;
-    extern __shared__ double2 smem[];
-    const int tx = threadIdx.x % XT;
-    const int tid = threadIdx.x / XT;
-    const int xtiles = mx / XT;
-    const unsigned bid = rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
-    const int ky = bid / xtiles, m = (bid % xtiles) * XT + tx;
-    const size_t stride = (size_t)mx * ny;
-    c2 *base = data + (size_t)ky * mx + m;
-    c2 x[E];
-#pragma unroll
-    for (int e = 0; e < E; ++e) x[e] = base[(size_t)(tid + e * T) * stride];
-    SmCol<XT> sm{smem + tx};
-    fft_line<L, E, -1, 1, SmCol<XT>>(x, tid, tw, sm);
-    const double exy = __ldg(&ex[m]) + __ldg(&ey[ky]);
-    const bool null_xy = (m == 0) && (((2 * ky) & (ny - 1)) == 0);
-#pragma unroll
-    for (int e = 0; e < E; ++e) {
-        const int kz = tid + e * T;
-        const double lam = -(exy + __ldg(&ez[kz]));
-        const bool null = null_xy && (((2 * kz) & (L - 1)) == 0);
-        const double s = null ? 0.0 : inv_n * __drcp_rn(lam);
-        x[e].x = null ? 0.0 : x[e].x * s;
-        x[e].y = null ? 0.0 : x[e].y * s;
-    }
-    fft_line<L, E, +1, 1, SmCol<XT>>(x, tid, tw, sm);
-#pragma unroll
-    for (int e = 0; e < E; ++e) base[(size_t)(tid + e * T) * stride] = x[e];
-}
-
 } // namespace dnsfft

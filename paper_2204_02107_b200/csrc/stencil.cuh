@@ -44,8 +44,8 @@ struct SourceDev {
     int off; // offset of this source's sx|sy|sz tables (nx+ny+nz doubles) in stab
 };
 
-// coefficients of the factored right-hand side used by k_rk_pair (host-computed, read from the constant bank)
-struct PairCoef {
+// coefficients of the factored right-hand side of k_rk_march (host-computed, read from the constant bank)
+struct RhsCoef {
     double hx, hy, hz;    // -1/(4 Delta_a)
     double dvx, dvy, dvz; // nu / Delta_a^2
     double dcx, dcy, dcz; // alpha_c / Delta_a^2
@@ -56,7 +56,6 @@ struct RKArgs {
     const double *qs[4]; // stage field (stencil input)
     const double *qn[4]; // Q^n
     const double *qc[4]; // running combination Qc, read (stages 2-4); with ELIM at stage 4: S = Q2 - Qn + 2 Q3
-    const double *q3[4]; // unused
     double *qo[4];       // next stage field, written (stages 1-3)
     double *qco[4];      // Qc written (accumulate form); with ELIM: S at stage 2, Q* at stage 4 (in place of S)
     const uint8_t *face; // null: no solid cells
@@ -70,7 +69,7 @@ struct RKArgs {
     int kc;                  // k_rk_march: planes per block
     int rev;                 // k_rk_march: walk the y tiles and z chunks from the far end (start on what the kernel before left in L2)
     const double *stab;
-    PairCoef kf;
+    RhsCoef kf;
     SourceDev src[DNS_MAX_SRC];
 };
 
@@ -321,9 +320,9 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
 #pragma unroll
             for (int m = 0; m < 4; ++m) qn[m] = cur[m];
         }
-        // factored form of the right-hand side (see k_rk_pair below): per cell six coefficients
+        // factored form of the right-hand side: per cell six coefficients shared by the four fields
         //   A+-_a = -(u_a(+-a) + u_a)/(4 Delta_a), then F = sum_a [q(+a)(A+_a + D_a) + q(-a)(D_a - A-_a)] - 2 sum_a D_a q0 + b
-        const PairCoef &kf = a.kf;
+        const RhsCoef &kf = a.kf;
         double axp[2], axm[2], ayp[2], aym[2], azp[2], azm[2];
         {
             const double2 vym = *reinterpret_cast<const double2 *>(sC + 1 * ROWS * SW + own - SW);
@@ -452,391 +451,6 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
         plane_step(t + 1, r1, r2, r0);
         if (t + 2 >= kc) break;
         plane_step(t + 2, r2, r0, r1);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// k_rk_pair: TWO Runge-Kutta stages per launch (stages 1+2, or 3+4), marching along z.
-//
-// Stage B of a pair needs the result of stage A only in a one-cell ring around the cell, so a block
-// that owns a 32 x 16 (x by y) column of cells evaluates stage A on the 34 x 18 region around it
-// (19.5 % redundant arithmetic) and keeps that result in shared memory; the intermediate stage field
-// never makes an HBM round trip.  Per step the four stages then move 28 field passes instead of 52:
-//   PAIR 0 (stages 1+2): read Qn;          Q2 = Qn + dt/2 F(Qn) stays on chip;
-//                        write Q3 = Qn + dt/2 F(Q2) and R = Q2 - Qn + 2 Q3                          (R4 W8)
-//   PAIR 1 (stages 3+4): read Q3, Qn, R;   Q4 = Qn + dt F(Q3) stays on chip;
-//                        write Q* = (R + Q4)/3 + dt/6 F(Q4), in place of R                          (R12 W4)
-// which is classical RK4: Q* = Qn + dt/6 (F1 + 2 F2 + 2 F3 + F4) with
-// F1 + 2 F2 + 2 F3 = (2 Q2 + 4 Q3 + 2 Q4 - 8 Qn)/dt.
-//
-// 320 threads, each owning TWO cells.  Threads 0..255: an x-adjacent, 16-byte aligned pair of interior
-// cells, in BOTH stages.  Threads 256..287: the pairs of the ring rows y0-1 and y0+16 (stage A only).
-// Threads 288..305: the two cells (x0-1, y) and (x0+32, y) of the ring columns (stage A only).
-// At iteration s the block
-//   - has the stage-A input planes a = k0-1+s (x/y neighbours) and a+1 (z+1 neighbour) in shared memory
-//     (cp.async, two more planes in flight: four plane tiles of 4 fields x 20 x 36 with the two-cell halo,
-//     periodic wrap applied to the source address); the z-1 neighbour and the centre ride in registers;
-//   - evaluates stage A at plane a into one of three A' tiles (4 fields x 18 x 36); in PAIR 1 the Qn plane it
-//     needs comes through three more tiles of that shape (cp.async, issued two iterations ahead);
-//   - evaluates stage B at plane b = a-1: centre, x/y and z-1 neighbours from the A' tiles written one and
-//     two iterations earlier, z+1 neighbour = this thread's own stage-A result of this iteration.
-// One __syncthreads per plane; the loop is unrolled three times so the z-carried registers and the tile
-// indices rotate by renaming.  F is evaluated in the factored form
-//   F = sum_a [ q(+a) (A+_a + D_a) + q(-a) (D_a - A-_a) ] - 2 (sum_a D_a) q0 + b,   A+-_a = -(u_a(+-a) + u_a)/(4 Delta_a),
-// which is the skew-symmetric form -1/2 [delta_a(u_a q) + u_a delta_a q] + D lap(q) term by term (same
-// value up to rounding; half the fp64 instructions of the literal form).
-constexpr int P2_TX = 32, P2_TY = 16, P2_NT = 320;
-constexpr int P2_W = P2_TX + 4;  // tile width, x0-2 .. x0+33; both tiles share this x origin so that pairs are 16-byte aligned
-constexpr int P2_QR = P2_TY + 4; // stage-A input tile rows, y0-2 .. y0+17
-constexpr int P2_AR = P2_TY + 2; // A' tile rows, y0-1 .. y0+16
-constexpr int P2_QF = P2_QR * P2_W, P2_AF = P2_AR * P2_W; // doubles per field per tile
-constexpr int P2_QPLANE = 4 * P2_QF, P2_APLANE = 4 * P2_AF;
-constexpr int P2_NQBUF = 4, P2_NABUF = 3;
-constexpr int P2_SMEM0 = (P2_NQBUF * P2_QPLANE + P2_NABUF * P2_APLANE) * (int)sizeof(double);     // PAIR 0
-constexpr int P2_SMEM1 = (P2_NQBUF * P2_QPLANE + 2 * P2_NABUF * P2_APLANE) * (int)sizeof(double); // PAIR 1: + three Qn tiles
-constexpr int P2_CHUNKS = P2_QR * (P2_W / 2);  // 16-byte chunks per field per stage-A input tile
-constexpr int P2_ACHUNKS = P2_AR * (P2_W / 2); // ... per A'-shaped (Qn) tile
-
-__device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
-
-
-typedef double pair4[4][2]; // [field][cell of the thread's pair]
-
-// x and y neighbours of the thread's two cells for one field (b = that field's tile, c = centre values)
-__device__ __forceinline__ void pair_nb(const double *b, int offL, int offR, bool split, const double (&c)[2], double (&xp)[2], double (&xm)[2],
-                                        double (&yp)[2], double (&ym)[2])
-{
-    if (!split) {
-        xm[0] = b[offL - 1];
-        xp[0] = c[1];
-        xm[1] = c[0];
-        xp[1] = b[offL + 2];
-        const double2 lo = *reinterpret_cast<const double2 *>(b + offL - P2_W), hi = *reinterpret_cast<const double2 *>(b + offL + P2_W);
-        ym[0] = lo.x; ym[1] = lo.y;
-        yp[0] = hi.x; yp[1] = hi.y;
-    } else {
-        xm[0] = b[offL - 1]; xp[0] = b[offL + 1];
-        xm[1] = b[offR - 1]; xp[1] = b[offR + 1];
-        ym[0] = b[offL - P2_W]; ym[1] = b[offR - P2_W];
-        yp[0] = b[offL + P2_W]; yp[1] = b[offR + P2_W];
-    }
-}
-
-// F for the four fields of the thread's two cells.  q0, zp, zm: centre and z neighbours (registers); the x
-// and y neighbours are read from `tile` (field stride FS) one field at a time, scalar first, so that few
-// values are live at once.
-template <bool MASKED, int FS>
-__device__ __forceinline__ void pair_rhs(const RKArgs &a, const PairCoef &k, const unsigned (&f)[2], const double *tile, int offL, int offR,
-                                         bool split, const pair4 &q0, const pair4 &zp, const pair4 &zm, pair4 &F)
-{
-    double axp[2], axm[2], ayp[2], aym[2], azp[2], azm[2];
-    {
-        double uxp[2], uxm[2], t0[2], t1[2], vyp[2], vym[2];
-        pair_nb(tile, offL, offR, split, q0[0], uxp, uxm, t0, t1);
-        pair_nb(tile + FS, offL, offR, split, q0[1], t0, t1, vyp, vym);
-#pragma unroll
-        for (int l = 0; l < 2; ++l) {
-            axp[l] = (uxp[l] + q0[0][l]) * k.hx; axm[l] = (uxm[l] + q0[0][l]) * k.hx;
-            ayp[l] = (vyp[l] + q0[1][l]) * k.hy; aym[l] = (vym[l] + q0[1][l]) * k.hy;
-            azp[l] = (zp[2][l] + q0[2][l]) * k.hz; azm[l] = (zm[2][l] + q0[2][l]) * k.hz;
-        }
-    }
-    {
-        double xp[2], xm[2], yp[2], ym[2];
-        pair_nb(tile + 3 * FS, offL, offR, split, q0[3], xp, xm, yp, ym);
-#pragma unroll
-        for (int l = 0; l < 2; ++l) {
-            double v;
-            if (!MASKED) {
-                v = k.dc0 * q0[3][l];
-                v = fma(xp[l], axp[l] + k.dcx, v);
-                v = fma(xm[l], k.dcx - axm[l], v);
-                v = fma(yp[l], ayp[l] + k.dcy, v);
-                v = fma(ym[l], k.dcy - aym[l], v);
-                v = fma(zp[3][l], azp[l] + k.dcz, v);
-                v = fma(zm[3][l], k.dcz - azm[l], v);
-            } else {
-                // eq. 4: no diffusive flux through solid faces (beta+- = beta * beta[+-1])
-                const unsigned fl = f[l];
-                const double exp_ = (fl & 2) ? k.dcx : 0.0, exm = (fl & 4) ? k.dcx : 0.0;
-                const double eyp = (fl & 8) ? k.dcy : 0.0, eym = (fl & 16) ? k.dcy : 0.0;
-                const double ezp = (fl & 32) ? k.dcz : 0.0, ezm = (fl & 64) ? k.dcz : 0.0;
-                v = -(((exp_ + exm) + (eyp + eym)) + (ezp + ezm)) * q0[3][l];
-                v = fma(xp[l], axp[l] + exp_, v);
-                v = fma(xm[l], exm - axm[l], v);
-                v = fma(yp[l], ayp[l] + eyp, v);
-                v = fma(ym[l], eym - aym[l], v);
-                v = fma(zp[3][l], azp[l] + ezp, v);
-                v = fma(zm[3][l], ezm - azm[l], v);
-            }
-            F[3][l] = v;
-        }
-    }
-#pragma unroll
-    for (int l = 0; l < 2; ++l) { // convective + viscous coefficients of the velocity components
-        axp[l] = axp[l] + k.dvx; axm[l] = k.dvx - axm[l];
-        ayp[l] = ayp[l] + k.dvy; aym[l] = k.dvy - aym[l];
-        azp[l] = azp[l] + k.dvz; azm[l] = k.dvz - azm[l];
-    }
-#pragma unroll
-    for (int m = 0; m < 3; ++m) {
-        double xp[2], xm[2], yp[2], ym[2];
-        pair_nb(tile + m * FS, offL, offR, split, q0[m], xp, xm, yp, ym);
-#pragma unroll
-        for (int l = 0; l < 2; ++l) {
-            double v = fma(k.dv0, q0[m][l], a.body[m]);
-            v = fma(xp[l], axp[l], v);
-            v = fma(xm[l], axm[l], v);
-            v = fma(yp[l], ayp[l], v);
-            v = fma(ym[l], aym[l], v);
-            v = fma(zp[m][l], azp[l], v);
-            v = fma(zm[m][l], azm[l], v);
-            F[m][l] = v;
-        }
-    }
-}
-
-// source relaxation terms of eqs. 2-3 for the thread's two cells; smask: sources
-// whose x and y factors are non-zero at either cell
-__device__ __forceinline__ void pair_sources(const RKArgs &a, unsigned smask, int iL, int iR, int j, int kz, const pair4 &q0, pair4 &F)
-{
-    while (smask) {
-        const int s = __ffs(smask) - 1;
-        smask &= smask - 1;
-        const double *tb = a.stab + a.src[s].off;
-        const double syz = __ldg(&tb[a.nx + a.ny + kz]) * __ldg(&tb[a.nx + j]);
-        if (syz == 0.0) continue;
-        const double Sv[2] = {__ldg(&tb[iL]) * syz, __ldg(&tb[iR]) * syz};
-        const uint32_t comps = a.src[s].comps;
-#pragma unroll
-        for (int l = 0; l < 2; ++l) {
-            if (Sv[l] == 0.0) continue;
-#pragma unroll
-            for (int m = 0; m < 4; ++m)
-                if (comps & (1u << m)) F[m][l] += Sv[l] * (a.src[s].set[m] - q0[m][l]) * a.src[s].rtau;
-        }
-    }
-}
-
-// the two cells' values of the four fields in a tile (field stride FS); PAIRED: one 16-byte access
-template <int FS> __device__ __forceinline__ void pair_ld(const double *tile, int offL, int offR, bool split, pair4 &v)
-{
-#pragma unroll
-    for (int m = 0; m < 4; ++m) {
-        if (!split) {
-            const double2 d = *reinterpret_cast<const double2 *>(tile + m * FS + offL);
-            v[m][0] = d.x;
-            v[m][1] = d.y;
-        } else {
-            v[m][0] = tile[m * FS + offL];
-            v[m][1] = tile[m * FS + offR];
-        }
-    }
-}
-
-template <int PAIR, bool MASKED, bool SOURCES> __global__ void __launch_bounds__(P2_NT, 1) k_rk_pair(const RKArgs a)
-{
-    extern __shared__ double2 p2_smem2[];
-    double *smQ = reinterpret_cast<double *>(p2_smem2);
-    double *smA = smQ + P2_NQBUF * P2_QPLANE;
-    double *smN = smA + P2_NABUF * P2_APLANE; // PAIR 1: Qn tiles
-    const int t = threadIdx.x;
-    const int nx = a.nx, ny = a.ny, nz = a.nz, kc = a.kc;
-    const int x0 = blockIdx.x * P2_TX, y0 = blockIdx.y * P2_TY, k0 = blockIdx.z * kc;
-    const size_t plane = (size_t)nx * ny;
-
-    // ---- this thread's two cells: A' tile row ar (y = y0-1+ar), tile columns colL, colR (x = x0-2+col)
-    const bool interior = t < 256;
-    const bool split = t >= 288;
-    const bool hasA = t < 288 + P2_AR;
-    int ar, colL, colR;
-    if (t < 256) {
-        ar = (t >> 4) + 1;
-        colL = 2 * (t & 15) + 2;
-        colR = colL + 1;
-    } else if (t < 288) {
-        ar = (t - 256) < 16 ? 0 : P2_AR - 1;
-        colL = 2 * (t & 15) + 2;
-        colR = colL + 1;
-    } else {
-        ar = (t - 288) < P2_AR ? (t - 288) : P2_AR - 1;
-        colL = 1;
-        colR = P2_W - 2;
-    }
-    const int gj = (y0 - 1 + ar) & (ny - 1), giL = (x0 - 2 + colL) & (nx - 1), giR = (x0 - 2 + colR) & (nx - 1);
-    const unsigned ocL = (unsigned)nx * gj + giL, ocR = (unsigned)nx * gj + giR; // offsets of the two columns inside a plane
-    const int qL = (ar + 1) * P2_W + colL, qR = (ar + 1) * P2_W + colR;    // inside a field of a stage-A input tile
-    const int aL = ar * P2_W + colL, aR = ar * P2_W + colR;                // inside a field of an A' (or Qn) tile
-
-    // ---- this thread's share of the plane tiles: up to two 16-byte chunks per field
-    const int lr0 = t / (P2_W / 2), lc0 = t - lr0 * (P2_W / 2);
-    const int t1 = t + P2_NT, lr1 = t1 / (P2_W / 2), lc1 = t1 - lr1 * (P2_W / 2);
-    const bool hasL1 = t1 < P2_CHUNKS, hasN0 = t < P2_ACHUNKS, hasN1 = t1 < P2_ACHUNKS;
-    const int lx0 = (x0 - 2 + 2 * lc0) & (nx - 1), lx1 = (x0 - 2 + 2 * lc1) & (nx - 1);
-    const unsigned ls0 = (unsigned)nx * ((y0 - 2 + lr0) & (ny - 1)) + lx0, ls1 = (unsigned)nx * ((y0 - 2 + lr1) & (ny - 1)) + lx1;
-    const unsigned ns0 = (unsigned)nx * ((y0 - 1 + lr0) & (ny - 1)) + lx0, ns1 = (unsigned)nx * ((y0 - 1 + lr1) & (ny - 1)) + lx1;
-    const int ld0 = lr0 * P2_W + 2 * lc0, ld1 = lr1 * P2_W + 2 * lc1;
-    // stage-A input plane k0-2+n into tile n % 4; PAIR 1: Qn at plane k0-1+sn (stage-A plane of iteration sn) into tile phn
-    auto issue_planes = [&](int n, bool doq, int sn, int phn, bool don) {
-        if (doq) {
-            const size_t pk = plane * (size_t)((k0 - 2 + n) & (nz - 1));
-            double *sb = smQ + (n & (P2_NQBUF - 1)) * P2_QPLANE;
-#pragma unroll
-            for (int m = 0; m < 4; ++m) {
-                cp_async16(sb + m * P2_QF + ld0, a.qs[m] + pk + ls0);
-                if (hasL1) cp_async16(sb + m * P2_QF + ld1, a.qs[m] + pk + ls1);
-            }
-        }
-        if (PAIR == 1 && don) {
-            const size_t pk = plane * (size_t)((k0 - 1 + sn) & (nz - 1));
-            double *sb = smN + phn * P2_APLANE;
-#pragma unroll
-            for (int m = 0; m < 4; ++m) {
-                if (hasN0) cp_async16(sb + m * P2_AF + ld0, a.qn[m] + pk + ns0);
-                if (hasN1) cp_async16(sb + m * P2_AF + ld1, a.qn[m] + pk + ns1);
-            }
-        }
-        cp_async_commit();
-    };
-
-    const PairCoef &kf = a.kf;
-
-    unsigned smask = 0;
-    if (SOURCES && hasA) {
-        for (int s = 0; s < a.nsrc; ++s) {
-            const double *tb = a.stab + a.src[s].off;
-            if ((__ldg(&tb[giL]) != 0.0 || __ldg(&tb[giR]) != 0.0) && __ldg(&tb[nx + gj]) != 0.0) smask |= 1u << s;
-        }
-    }
-
-    issue_planes(1, true, 0, 0, true);
-    issue_planes(2, true, 1, 1, true);
-    issue_planes(3, true, 0, 0, false);
-
-    // face bytes of the two cells, fetched one iteration ahead and left packed until they are used
-    auto ld_face = [&](size_t pk, unsigned (&raw)[2]) {
-        if (!split) {
-            raw[0] = *reinterpret_cast<const unsigned short *>(a.face + pk + ocL);
-        } else {
-            raw[0] = a.face[pk + ocL];
-            raw[1] = a.face[pk + ocR];
-        }
-    };
-
-    // z-carried registers: three rotating sets for the stage-A input column
-    pair4 R0, R1, R2;
-    unsigned fA[2] = {0x7f, 0x7f}, fB[2] = {0x7f, 0x7f}, fN[2] = {0x7f7f, 0x7f};
-#pragma unroll
-    for (int m = 0; m < 4; ++m)
-#pragma unroll
-        for (int l = 0; l < 2; ++l) R0[m][l] = R1[m][l] = R2[m][l] = 0.0;
-    if (hasA) {
-        const size_t pm2 = plane * (size_t)((k0 - 2) & (nz - 1)), pm1 = plane * (size_t)((k0 - 1) & (nz - 1));
-#pragma unroll
-        for (int m = 0; m < 4; ++m) {
-            if (!split) {
-                const double2 d = *reinterpret_cast<const double2 *>(a.qs[m] + pm2 + ocL);
-                R0[m][0] = d.x;
-                R0[m][1] = d.y;
-            } else {
-                R0[m][0] = a.qs[m][pm2 + ocL];
-                R0[m][1] = a.qs[m][pm2 + ocR];
-            }
-        }
-        if (MASKED) ld_face(pm1, fN);
-    }
-
-    // one plane: stage A at plane k0-1+s, stage B at plane k0-2+s.  ph = s % 3 (A' and Qn tile rotation)
-    auto body = [&](const int s, const int ph, pair4 &Azm, pair4 &Ac, pair4 &Azp) {
-        const int ka = (k0 - 1 + s) & (nz - 1), kb = (ka - 1) & (nz - 1);
-        fB[0] = fA[0]; fB[1] = fA[1];
-        fA[0] = split ? fN[0] : (fN[0] & 0xffu);
-        fA[1] = split ? fN[1] : (fN[0] >> 8);
-        if (MASKED && hasA && s <= kc) ld_face(plane * (size_t)((ka + 1) & (nz - 1)), fN);
-        double2 rb[4]; // PAIR 1: R at the stage-B plane, consumed at the very end of the iteration
-        if (PAIR == 1 && interior && s >= 2) {
-#pragma unroll
-            for (int m = 0; m < 4; ++m) rb[m] = *reinterpret_cast<const double2 *>(a.qc[m] + plane * (size_t)kb + ocL);
-        }
-
-        cp_async_wait_1();
-        __syncthreads(); // tiles of this iteration visible; every thread is done with iteration s-1
-        issue_planes(s + 4, s + 4 <= kc + 3, s + 2, (ph + 2) % 3, s + 2 <= kc + 1);
-
-        const double *sQ = smQ + ((s + 1) & (P2_NQBUF - 1)) * P2_QPLANE;
-        const double *sZ = smQ + ((s + 2) & (P2_NQBUF - 1)) * P2_QPLANE;
-        double *sAw = smA + ph * P2_APLANE;                        // A'(a), written now
-        const double *sAc = smA + ((ph + 2) % 3) * P2_APLANE;      // A'(b)   = A'(a-1)
-        const double *sAm = smA + ((ph + 1) % 3) * P2_APLANE;      // A'(b-1) = A'(a-2)
-        const double *sN = smN + ph * P2_APLANE;                   // PAIR 1: Qn(a)
-
-        // ---- stage A at plane ka
-        pair4 Aout;
-        if (hasA) {
-            if (s == 0) pair_ld<P2_QF>(sQ, qL, qR, split, Ac);
-            pair_ld<P2_QF>(sZ, qL, qR, split, Azp);
-        }
-        if (hasA && (interior || (s >= 1 && s <= kc))) { // ring cells feed stage B only at planes k0..k0+kc-1
-            pair4 F;
-            pair_rhs<MASKED, P2_QF>(a, kf, fA, sQ, qL, qR, split, Ac, Azp, Azm, F);
-            if (SOURCES) pair_sources(a, smask, giL, giR, gj, ka, Ac, F);
-            pair4 base;
-            if (PAIR == 1) pair_ld<P2_AF>(sN, aL, aR, split, base);
-#pragma unroll
-            for (int m = 0; m < 4; ++m) {
-#pragma unroll
-                for (int l = 0; l < 2; ++l) {
-                    // solid cell: every field it holds is +0.0 and stays +0.0 (select)
-                    const bool fl = !MASKED || (fA[l] & 1);
-                    Aout[m][l] = fl ? (PAIR == 0 ? Ac[m][l] : base[m][l]) + a.ca * F[m][l] : 0.0;
-                }
-                if (!split) {
-                    *reinterpret_cast<double2 *>(sAw + m * P2_AF + aL) = make_double2(Aout[m][0], Aout[m][1]);
-                } else {
-                    sAw[m * P2_AF + aL] = Aout[m][0];
-                    sAw[m * P2_AF + aR] = Aout[m][1];
-                }
-            }
-        }
-
-        // ---- stage B at plane kb = ka-1: centre, x/y and z-1 neighbours from the A' tiles of the last two
-        //      iterations, z+1 neighbour = this thread's own stage-A result of this iteration
-        if (interior && s >= 2) {
-            pair4 Bc, Bzm, F;
-            pair_ld<P2_AF>(sAc, aL, aR, false, Bc);
-            pair_ld<P2_AF>(sAm, aL, aR, false, Bzm);
-            pair_rhs<MASKED, P2_AF>(a, kf, fB, sAc, aL, aR, false, Bc, Aout, Bzm, F);
-            if (SOURCES) pair_sources(a, smask, giL, giR, gj, kb, Bc, F);
-            const size_t o = plane * (size_t)kb + ocL;
-            const bool flx = !MASKED || (fB[0] & 1), fly = !MASKED || (fB[1] & 1);
-#pragma unroll
-            for (int m = 0; m < 4; ++m) {
-                double2 q, r;
-                if (PAIR == 0) {
-                    // Azm = Qn(b), Bc = Q2(b):  Q3 = Qn + dt/2 F(Q2),  R = Q2 - Qn + 2 Q3
-                    const double q3x = Azm[m][0] + a.cb * F[m][0], q3y = Azm[m][1] + a.cb * F[m][1];
-                    q.x = flx ? q3x : 0.0;
-                    q.y = fly ? q3y : 0.0;
-                    r.x = flx ? (Bc[m][0] - Azm[m][0]) + 2.0 * q3x : 0.0;
-                    r.y = fly ? (Bc[m][1] - Azm[m][1]) + 2.0 * q3y : 0.0;
-                    *reinterpret_cast<double2 *>(a.qco[m] + o) = q;
-                    *reinterpret_cast<double2 *>(a.qo[m] + o) = r;
-                } else {
-                    // Bc = Q4(b):  Q* = (R + Q4)/3 + dt/6 F(Q4)
-                    q.x = flx ? (rb[m].x + Bc[m][0]) * (1.0 / 3.0) + a.cb * F[m][0] : 0.0;
-                    q.y = fly ? (rb[m].y + Bc[m][1]) * (1.0 / 3.0) + a.cb * F[m][1] : 0.0;
-                    *reinterpret_cast<double2 *>(a.qco[m] + o) = q;
-                }
-            }
-        }
-    };
-
-    for (int s = 0; s <= kc + 1; s += 3) {
-        body(s, 0, R0, R1, R2);
-        if (s + 1 > kc + 1) break;
-        body(s + 1, 1, R1, R2, R0);
-        if (s + 2 > kc + 1) break;
-        body(s + 2, 2, R2, R0, R1);
     }
 }
 

@@ -37,7 +37,8 @@ def test_workspace_bytes_validates(L):
     assert w >= 19 * 8 * n + n and w % 256 == 0
     assert binding.workspace_bytes(binding.make_params((16, 32, 64), (0.1, 0.1, 0.1), 1e-3, 1e-3, 1e-2, flags=2)) >= w + 8 * n
     bad = [dict(shape=(16, 32, 48)), dict(shape=(4, 32, 64)), dict(shape=(16, 2048, 64)), dict(shape=(16, 32, 4096)),
-           dict(d=(0.0, 0.1, 0.1)), dict(dt=0.0), dict(nu=-1.0), dict(n_piter=0), dict(flags=16), dict(dt=float("nan"))]
+           dict(d=(0.0, 0.1, 0.1)), dict(dt=0.0), dict(nu=-1.0), dict(n_piter=0), dict(flags=4), dict(flags=8), dict(flags=16),
+           dict(dt=float("nan"))]
     for b in bad:
         kw = dict(shape=(16, 32, 64), d=(0.1, 0.1, 0.1), nu=1e-3, alpha_c=1e-3, dt=1e-2, n_piter=1, flags=0)
         kw.update(b)

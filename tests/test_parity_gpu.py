@@ -117,27 +117,46 @@ def test_config5_three_rooms_eighth_size_20_steps():
         compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"rooms/8 step {cp}")
 
 
-@pytest.mark.slow
-def test_config3_full_size_one_step():
-    case = cases.config(3)
-    for cp, got, ref in run_both(case, [1]):
-        compare(got, ref, TOL1, what="turb256 step 1")
+# Full-size cases (north_star: "all five configs match the CPU oracle"; compare at steps 1 and 100).
+# The measured errors are recorded by the tests themselves in the `record_property` of the junit log and tabulated in
+# DESIGN.md section 3 from the log kept under profiles/.
+def _full_size(case, checkpoints, record_property, what):
+    for cp, got, ref in run_both(case, checkpoints):
+        errs = {k: relerr(got[k], ref[k]) for k in "uvwcp"}
+        record_property(f"{what} step {cp}", " ".join(f"{k}={e:.2e}" for k, e in errs.items()))
+        print(f"[parity] {what} step {cp}: " + " ".join(f"{k}={e:.2e}" for k, e in errs.items()), flush=True)
+        compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"{what} step {cp}")
 
 
 @pytest.mark.slow
-def test_config4_full_size_one_step():
-    case = cases.config(4)
-    for cp, got, ref in run_both(case, [1]):
-        compare(got, ref, TOL1, mask=case["mask"], what="room512 step 1")
+def test_config3_full_size_100_steps(record_property):
+    _full_size(cases.config(3), [1, 100], record_property, "config 3, 256^3")
 
 
 @pytest.mark.slow
-def test_config5_half_size_one_step():
-    """Config 5's generator (three rooms, doorways, two ducts, 30 boxes) at 512x256x128 -- the largest size at which the
-    oracle still finishes a step in seconds (full size: 134 M cells, 22 GB and minutes per oracle step)."""
-    case = cases.config(5, shrink=2)
-    for cp, got, ref in run_both(case, [1]):
-        compare(got, ref, TOL1, mask=case["mask"], what="rooms/2 step 1")
+def test_config4_full_size_100_steps(record_property):
+    """The bench headline workload: 512x256x128 room, P = 4, steps 1 and 100."""
+    _full_size(cases.config(4), [1, 100], record_property, "config 4, 512x256x128")
+
+
+@pytest.mark.slow
+def test_config5_half_size_100_steps(record_property):
+    """Config 5's generator (three rooms, doorways, two ducts, 30 boxes) at 512x256x128, steps 1 and 100."""
+    _full_size(cases.config(5, shrink=2), [1, 100], record_property, "config 5 at half size, 512x256x128")
+
+
+@pytest.mark.slow
+def test_config5_full_size_one_step(record_property):
+    """1024x512x256 (134 M cells): the oracle holds 21 fields of 1.07 GB, the case 5 more, the comparison 10 more --
+    about 40 GB of host memory.  If the box has less than 64 GB available the z extent is halved (and the test says
+    so in its record); the FFT lines along x and y keep their full length either way."""
+    import psutil
+    avail = psutil.virtual_memory().available / 2 ** 30
+    if avail >= 64:
+        case, what = cases.config(5), "config 5, 1024x512x256"
+    else:
+        case, what = cases.three_rooms(1024, 512, 128), f"config 5 z-halved to 1024x512x128 ({avail:.0f} GB host RAM available)"
+    _full_size(case, [1], record_property, what)
 
 
 # ------------------------------------------------------------------ variants and edge cases
@@ -149,10 +168,9 @@ def test_per_stage_projection_variant():
 
 def test_eq6_filter_variant():
     """NEXT-1, flags bit 0: eq. 6 filter on u, v, w, c at the end of every step (masked room with sources, periodic
-    box, with per-stage projection, with the two-stage RK kernel, and a grid thinner than the stencil is wide)."""
+    box, with per-stage projection, and a grid thinner than the stencil is wide)."""
     for case, cps, flags in [(cases.duct_room(64, 32, 32), [1, 20], 1), (cases.periodic_turbulence(32, steps=5), [1, 5], 1),
-                             (cases.duct_room(32, 16, 16), [1, 5], 3), (cases.duct_room(64, 32, 32), [1, 5], 9),
-                             (cases.duct_room(32, 8, 8), [1, 3], 1)]:
+                             (cases.duct_room(32, 16, 16), [1, 5], 3), (cases.duct_room(32, 8, 8), [1, 3], 1)]:
         for cp, got, ref in run_both(case, cps, flags=flags):
             compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"flags={flags} {case['name']} step {cp}")
     case = cases.duct_room(64, 32, 32)
@@ -253,40 +271,27 @@ def test_next4_lagrangian_particles():
         s.close()
 
 
-def test_two_stage_rk_kernel_variant():
-    """flags bit 3: stages 1+2 and 3+4 fused (k_rk_pair, intermediate stage field in shared memory) -- same method,
-    same tolerances; masked with sources, unmasked, a grid of one tile in x, and a z extent of one chunk."""
-    for case, cps in [(cases.duct_room(64, 32, 32), [1, 20]), (cases.config(1), [1, 10]), (cases.duct_room(32, 16, 8), [1, 3])]:
-        for cp, got, ref in run_both(case, cps, flags=8):
-            compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"flags=8 {case['name']} step {cp}")
-    case = cases.duct_room(64, 32, 32)
-    s = binding.solver_for_case(case, flags=8)
-    n0 = s.launch_count()
-    s.step(1)
-    assert s.launch_count() - n0 == 2 + 1 + 4 * 6 + 1
-    s.close()
-
-
 def test_eq9_sparse_list_and_dense_prologue_agree():
-    """eq. 9's right-hand side at the listed near-solid cells (default) and densely inside the forward x pass
-    (flags bit 2) are the same arithmetic: both match the oracle, and each other to rounding."""
-    case = cases.duct_room(64, 32, 32)
-    res = {}
-    for flags in (0, 4):
-        s = binding.solver_for_case(case, flags=flags)
+    """eq. 9's right-hand side is evaluated at the listed near-solid cells (one extra launch per iteration) when they
+    are at most half of the grid, and densely inside the forward x pass otherwise (the library decides; same
+    arithmetic).  A room (9 % near-solid) takes the first path, a random mask with 35 % solid cells the second;
+    both match the oracle."""
+    rng = np.random.default_rng(12)
+    room = cases.duct_room(64, 32, 32)
+    dense = dict(room, sources=[])
+    dense["mask"] = (rng.random(room["shape"]) > 0.35).astype(np.uint8)
+    for k in "uvwc":
+        dense[k] = room[k] + 1e-3 * rng.standard_normal(room["shape"])
+    for case, per_iter in ((room, 6), (dense, 5)):
+        s = binding.solver_for_case(case)
         n0 = s.launch_count()
         s.step(3)
-        per_step = (s.launch_count() - n0) // 3
-        assert per_step == (4 + 1 + 4 * 6 + 1 if flags == 0 else 4 + 1 + 4 * 5 + 1)   # sparse: +1 launch per iteration
-        res[flags] = s.fields_numpy()
+        assert (s.launch_count() - n0) // 3 == 4 + 1 + 4 * per_iter + 1, case["name"]
+        got = s.fields_numpy()
         s.close()
-    o = oracle_for(case)
-    o.step(3)
-    ref = o.fields()
-    for flags in (0, 4):
-        compare(res[flags], ref, TOL1, mask=case["mask"], what=f"eq9 flags={flags}")
-    for k in "uvwcp":
-        assert relerr(res[0][k], res[4][k]) <= 1e-13
+        o = oracle_for(case)
+        o.step(3)
+        compare(got, o.fields(), TOL1, mask=case["mask"], what=f"eq9 {per_iter} launches per iteration")
 
 
 def test_smooth_tanh_sources_and_body_force_unequal_spacing():
@@ -376,6 +381,9 @@ def test_create_rejects_bad_arguments():
     assert L.dnslab_create(C.byref(P), None, None, 3, base, None, C.byref(h)) == -1          # nsrc without src
     bad = binding.make_sources([dict(lo=(0, 0, 0), size=(1, 1, 1), tau_f=0.0)])
     assert L.dnslab_create(C.byref(P), None, bad, 1, base, None, C.byref(h)) == -1           # tau_f <= 0
+    for size in ((0, 1, 1), (1, 9, 1), (1, 1, -2)):
+        bad = binding.make_sources([dict(lo=(0, 0, 0), size=size, tau_f=1.0, B=(1.0, 1.0, 1.0))])
+        assert L.dnslab_create(C.byref(P), None, bad, 1, base, None, C.byref(h)) == -1       # size outside 1..N
     assert L.dnslab_create(C.byref(P), None, None, 0, base, None, C.byref(h)) == 0
     assert L.dnslab_step(h, -1) == -1
     assert L.dnslab_poisson(h, None, None) == -1
