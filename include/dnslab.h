@@ -127,7 +127,9 @@ int64_t dnslab_launch_count(const dnslab_t *h);
 #define DNSLAB_K_FILTER 7  /* eq. 6 filter (flags bit 0)                                    */
 #define DNSLAB_K_REDUCE 8  /* Courant-number and scalar mean/std reductions (NEXT-3)         */
 #define DNSLAB_K_PARTICLES 9 /* Lagrangian particle step (NEXT-4)                             */
-#define DNSLAB_NCLASS 10
+#define DNSLAB_K_FFT_XY 10   /* two-pass solve: x and the high digit of y in one pass (forward, inverse) */
+#define DNSLAB_K_FFT_YZ 11   /* two-pass solve: low digit of y, z forward, division, and back             */
+#define DNSLAB_NCLASS 12
 int dnslab_profile(dnslab_t *h, int enable);
 int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches);
 

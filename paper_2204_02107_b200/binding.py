@@ -13,7 +13,8 @@ LIB_PATH = os.path.join(_HERE, "libdnslab.so")
 SYMBOLS = ["dnslab_workspace_bytes", "dnslab_create", "dnslab_set_fields", "dnslab_step", "dnslab_poisson",
            "dnslab_fields", "dnslab_get_fields", "dnslab_launch_count", "dnslab_profile", "dnslab_profile_read",
            "dnslab_courant", "dnslab_set_dt", "dnslab_scalar_stats", "dnslab_particles_attach", "dnslab_destroy", "dnslab_strerror"]
-KERNEL_CLASSES = ["rk_stage", "div", "fft_x", "fft_y", "fft_z_solve", "project", "eq9_sparse", "filter", "reduce", "particles"]
+KERNEL_CLASSES = ["rk_stage", "div", "fft_x", "fft_y", "fft_z_solve", "project", "eq9_sparse", "filter", "reduce", "particles",
+                  "fft_xy", "fft_yz_solve"]
 
 
 class Params(C.Structure):

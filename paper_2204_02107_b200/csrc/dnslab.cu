@@ -40,7 +40,7 @@ bool valid_params(const dnslab_params_t *P)
 }
 
 struct Layout {
-    size_t field_bytes, off_fields, nfields, off_face, off_tw[3], off_eig, off_stab, off_blist, off_bsave, bcap, total;
+    size_t field_bytes, off_fields, nfields, off_face, off_tw[3], off_twy1, off_eig, off_stab, off_blist, off_bsave, bcap, total;
 };
 
 // 19 fields: Q(4) A(4) B(4) Qc(4) p d W (+1 scratch pressure with per-stage projection)
@@ -60,6 +60,8 @@ Layout make_layout(const dnslab_params_t *P)
         L.off_tw[a] = off;
         off += align_up((size_t)len[a] * sizeof(c2));
     }
+    L.off_twy1 = off; // twiddles of the inner y transform of the two-pass solve (at most 128 entries)
+    off += align_up(128 * sizeof(c2));
     L.off_eig = off;
     off += align_up((size_t)(P->nx / 2 + P->ny + P->nz) * sizeof(double));
     L.off_stab = off;
@@ -68,7 +70,7 @@ Layout make_layout(const dnslab_params_t *P)
     // list would be longer than N/2 use the dense prologue of the forward x pass instead
     L.bcap = n / 2;
     L.off_blist = off;
-    off += align_up(L.bcap * sizeof(uint32_t));
+    off += align_up(L.bcap * sizeof(uint64_t));
     L.off_bsave = off;
     off += align_up(L.bcap * sizeof(double));
     L.total = off;
@@ -106,10 +108,12 @@ struct dnslab {
     Layout L;
     double *Q[4], *A[4], *Bf[4], *Qc[4], *p, *d, *W, *ps;
     uint8_t *face; // null when the mask has no solid cell
-    uint32_t *blist; // eq. 9 boundary list; null: dense prologue in the forward x pass
+    unsigned long long *blist; // eq. 9 boundary records (index | face << 32); null: dense prologue in the forward x pass
     double *bsave;
     int nb;
     c2 *tw[3];
+    c2 *twy1;  // exp(-2 pi i t/NY1), the inner y transform of the two-pass solve
+    int f_ny1; // two-pass solve (k_fft_xy + k_fft_yz_solve): rows per xy tile, 0 = five single-axis passes instead
     double *eig[3];
     double *stab;
     int nsrc;
@@ -381,6 +385,90 @@ int launch_fft_z_solve(dnslab *h, c2 *data)
     return DNSLAB_EINVAL;
 }
 
+// ---- two-pass solve: k_fft_xy (x and the high digit of y) and k_fft_yz_solve (low digit of y, z, division) --------
+// A tile of the xy pass is 8192 complex numbers (NY1 = 8192 / (nx/2) whole rows, 144 KB of shared memory with padding);
+// the fused middle pass takes NY0 = ny / NY1 rows by all of z for XT adjacent kx, at most 8192 numbers again.
+// Shapes outside these limits (and masks that need the dense eq. 9 prologue) use the five single-axis passes.
+constexpr int XY_TILE = 8192;
+
+int fused_ny1(const dnslab_params_t *P)
+{
+    const int mx = P->nx / 2;
+    if (mx < 64 || mx > 512) return 0;
+    const int ny1 = XY_TILE / mx; // 128, 64, 32, 16
+    if (P->ny < ny1) return 0;
+    const int ny0 = P->ny / ny1;
+    if (ny0 == 1) return ny1; // the middle pass is then the plain fused z pass
+    if (ny0 > 16 || P->nz < 32 || ny0 * P->nz > 2048) return 0;
+    return ny1;
+}
+
+template <int LX, int DIR> int launch_fft_xy_L(dnslab *h, const c2 *in, c2 *out)
+{
+    constexpr int NY1 = XY_TILE / LX, NT = XY_TILE / 16;
+    const size_t smem = (size_t)NY1 * (LX + LX / 8) * sizeof(c2);
+    auto kern = dnsfft::k_fft_xy<LX, NY1, DIR>;
+    if (h->prepare) {
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        return DNSLAB_OK;
+    }
+    ProfScope ps(h, DNSLAB_K_FFT_XY);
+    kern<<<(unsigned)((h->P.ny / NY1) * h->P.nz), NT, smem, h->stream>>>(in, out, h->tw[0], h->twy1, h->tw[1], h->P.ny, DIR < 0 ? 0 : 1);
+    return check_launch(h);
+}
+
+template <int DIR> int launch_fft_xy(dnslab *h, const c2 *in, c2 *out)
+{
+    switch (h->P.nx / 2) {
+    case 64: return launch_fft_xy_L<64, DIR>(h, in, out);
+    case 128: return launch_fft_xy_L<128, DIR>(h, in, out);
+    case 256: return launch_fft_xy_L<256, DIR>(h, in, out);
+    case 512: return launch_fft_xy_L<512, DIR>(h, in, out);
+    }
+    return DNSLAB_EINVAL;
+}
+
+template <int NY0, int LZ> int launch_fft_yz_solve_NL(dnslab *h, c2 *data)
+{
+    constexpr int XT = (XY_TILE / (NY0 * LZ)) > 16 ? 16 : XY_TILE / (NY0 * LZ), NT = XT * NY0 * LZ / 16;
+    const size_t smem = (size_t)XT * NY0 * LZ * sizeof(c2);
+    auto kern = dnsfft::k_fft_yz_solve<NY0, LZ, XT>;
+    if (h->prepare) {
+        if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        return DNSLAB_OK;
+    }
+    const int mx = h->P.nx / 2;
+    ProfScope ps(h, DNSLAB_K_FFT_YZ);
+    kern<<<(unsigned)((mx / XT) * (h->P.ny / NY0)), NT, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2],
+                                                                          2.0 / (double)h->n, 1);
+    return check_launch(h);
+}
+
+template <int NY0> int launch_fft_yz_solve_N(dnslab *h, c2 *data)
+{
+    switch (h->P.nz) {
+    case 32: return launch_fft_yz_solve_NL<NY0, 32>(h, data);
+    case 64: return launch_fft_yz_solve_NL<NY0, 64>(h, data);
+    case 128: return launch_fft_yz_solve_NL<NY0, 128>(h, data);
+    case 256: if constexpr (NY0 <= 8) return launch_fft_yz_solve_NL<NY0, 256>(h, data); break;
+    case 512: if constexpr (NY0 <= 4) return launch_fft_yz_solve_NL<NY0, 512>(h, data); break;
+    case 1024: if constexpr (NY0 <= 2) return launch_fft_yz_solve_NL<NY0, 1024>(h, data); break;
+    }
+    return DNSLAB_EINVAL;
+}
+
+int launch_fft_yz_solve(dnslab *h, c2 *data)
+{
+    switch (h->P.ny / h->f_ny1) {
+    case 1: return launch_fft_z_solve(h, data);
+    case 2: return launch_fft_yz_solve_N<2>(h, data);
+    case 4: return launch_fft_yz_solve_N<4>(h, data);
+    case 8: return launch_fft_yz_solve_N<8>(h, data);
+    case 16: return launch_fft_yz_solve_N<16>(h, data);
+    }
+    return DNSLAB_EINVAL;
+}
+
 // One solve p = F^-1[F[r]/lambda]; r = eq. 9 right-hand side built from (d, pold, face) on the fly
 // when `prologue`, else r = d as given.  pout may alias d or pold (it is written by the last pass).
 int poisson_solve(dnslab *h, const double *d, const double *pold, double *pout, bool prologue)
@@ -392,6 +480,11 @@ int poisson_solve(dnslab *h, const double *d, const double *pold, double *pout, 
     ra.r2x = 1.0 / (2.0 * h->P.dx); ra.r2y = 1.0 / (2.0 * h->P.dy); ra.r2z = 1.0 / (2.0 * h->P.dz);
     c2 *W = reinterpret_cast<c2 *>(h->W);
     int rc;
+    if (!prologue && h->f_ny1 > 0) {
+        if ((rc = launch_fft_xy<-1>(h, reinterpret_cast<const c2 *>(d), W))) return rc;
+        if ((rc = launch_fft_yz_solve(h, W))) return rc;
+        return launch_fft_xy<+1>(h, W, reinterpret_cast<c2 *>(pout));
+    }
     if (prologue) rc = launch_fft_x<-1, true>(h, reinterpret_cast<const c2 *>(d), W, ra);
     else rc = launch_fft_x<-1, false>(h, reinterpret_cast<const c2 *>(d), W, ra);
     if (rc) return rc;
@@ -443,8 +536,8 @@ int launch_eq9_sparse(dnslab *h, const double *p, bool first)
     const int per = 256 * dnsst::EQ9_ITEMS;
     const unsigned grid = (unsigned)((h->nb + per - 1) / per);
     const double r2x = 1.0 / (2.0 * h->P.dx), r2y = 1.0 / (2.0 * h->P.dy), r2z = 1.0 / (2.0 * h->P.dz);
-    if (first) dnsst::k_eq9_sparse<true><<<grid, 256, 0, h->stream>>>(h->d, p, h->face, h->blist, h->bsave, h->nb, h->P.nx, h->P.ny, h->P.nz, lgx, lgy, r2x, r2y, r2z);
-    else dnsst::k_eq9_sparse<false><<<grid, 256, 0, h->stream>>>(h->d, p, h->face, h->blist, h->bsave, h->nb, h->P.nx, h->P.ny, h->P.nz, lgx, lgy, r2x, r2y, r2z);
+    if (first) dnsst::k_eq9_sparse<true><<<grid, 256, 0, h->stream>>>(h->d, p, h->blist, h->bsave, h->nb, h->P.nx, h->P.ny, h->P.nz, lgx, lgy, r2x, r2y, r2z);
+    else dnsst::k_eq9_sparse<false><<<grid, 256, 0, h->stream>>>(h->d, p, h->blist, h->bsave, h->nb, h->P.nx, h->P.ny, h->P.nz, lgx, lgy, r2x, r2y, r2z);
     return check_launch(h);
 }
 
@@ -535,6 +628,7 @@ int prepare_kernels(dnslab *h)
         if ((rc = launch_rk<4, true>(h, h->A, nullptr, h->Qc))) return rc;
     }
     if ((rc = poisson_solve(h, h->d, h->p, h->p, true))) return rc;
+    if ((rc = poisson_solve(h, h->d, h->p, h->p, false))) return rc; // dnslab_poisson: never the dense prologue
     if ((h->P.flags & 1u) && (rc = launch_filter(h, h->Qc, h->A))) return rc;
     return DNSLAB_OK;
 }
@@ -641,7 +735,7 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
         if (any_solid) {
             // cells with at least one solid face neighbour, ascending index order
             const int nx = params->nx, ny = params->ny, nz = params->nz;
-            std::vector<uint32_t> bl;
+            std::vector<unsigned long long> bl;
             bool fits = true;
             for (int k = 0; k < nz && fits; ++k) {
                 const size_t kp = (size_t)((k + 1) & (nz - 1)), km = (size_t)((k - 1) & (nz - 1));
@@ -651,17 +745,19 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
                     const uint8_t *ryp = hm.data() + (size_t)nx * (jp + (size_t)ny * k), *rym = hm.data() + (size_t)nx * (jm + (size_t)ny * k);
                     const uint8_t *rzp = hm.data() + (size_t)nx * (j + (size_t)ny * kp), *rzm = hm.data() + (size_t)nx * (j + (size_t)ny * km);
                     for (int i = 0; i < nx; ++i) {
-                        if (r0[(i + 1) & (nx - 1)] && r0[(i - 1) & (nx - 1)] && ryp[i] && rym[i] && rzp[i] && rzm[i]) continue;
+                        const unsigned f = (r0[i] != 0) | ((r0[(i + 1) & (nx - 1)] != 0) << 1) | ((r0[(i - 1) & (nx - 1)] != 0) << 2) |
+                                           ((ryp[i] != 0) << 3) | ((rym[i] != 0) << 4) | ((rzp[i] != 0) << 5) | ((rzm[i] != 0) << 6);
+                        if ((f & 0x7e) == 0x7e) continue; // all six neighbours fluid: the bracket is exactly 0
                         if (bl.size() >= L.bcap) { fits = false; break; }
-                        bl.push_back((uint32_t)((size_t)i + (size_t)nx * (j + (size_t)ny * k)));
+                        bl.push_back((unsigned long long)((size_t)i + (size_t)nx * (j + (size_t)ny * k)) | ((unsigned long long)f << 32));
                     }
                 }
             }
             if (fits) {
-                h->blist = (uint32_t *)(h->ws + L.off_blist);
+                h->blist = (unsigned long long *)(h->ws + L.off_blist);
                 h->bsave = (double *)(h->ws + L.off_bsave);
                 h->nb = (int)bl.size();
-                if (h->nb) CKF(cudaMemcpyAsync(h->blist, bl.data(), bl.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, h->stream));
+                if (h->nb) CKF(cudaMemcpyAsync(h->blist, bl.data(), bl.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, h->stream));
                 CKF(cudaStreamSynchronize(h->stream));
             }
         }
@@ -693,6 +789,19 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
             CKF(cudaMemcpyAsync(h->eig[a], e.data(), e.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
             CKF(cudaStreamSynchronize(h->stream));
         }
+    }
+
+    h->f_ny1 = fused_ny1(params);
+    h->twy1 = (c2 *)(h->ws + L.off_twy1);
+    if (h->f_ny1 > 0) {
+        std::vector<c2> tw(h->f_ny1);
+        for (int t = 0; t < h->f_ny1; ++t) {
+            const long double ang = -2.0L * 3.141592653589793238462643383279502884L * (long double)t / (long double)h->f_ny1;
+            tw[t].x = (double)cosl(ang);
+            tw[t].y = (double)sinl(ang);
+        }
+        CKF(cudaMemcpyAsync(h->twy1, tw.data(), tw.size() * sizeof(c2), cudaMemcpyHostToDevice, h->stream));
+        CKF(cudaStreamSynchronize(h->stream));
     }
 
     // sources: one-dimensional factor tables of eq. 5

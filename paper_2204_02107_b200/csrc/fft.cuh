@@ -390,4 +390,167 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 
     }
 }
 
+// ---------------------------------------------------------------------------------------
+// Two-pass transform (3 HBM round trips per solve instead of 5).  The y transform is split by Cooley-Tukey,
+// y = y0 + NY0 y1, ky = ky1 + NY1 ky0 (NY0 NY1 = ny):
+//     Y[ky1 + NY1 ky0] = sum_y0 w_NY0^(y0 ky0) { w_ny^(y0 ky1) [ sum_y1 f[y0 + NY0 y1] w_NY1^(y1 ky1) ] } .
+// k_fft_xy does x and the inner sum (over y1) plus the twiddle on a tile of NY1 whole rows y0 + NY0 y1 (each row is
+// LX contiguous complex numbers) and leaves ky1 where y1 was; k_fft_yz_solve does the outer sum (over y0: NY0
+// adjacent rows), z, the division by lambda(kx, ky1 + NY1 ky0, kz), and the way back.  Frequencies stay in this
+// digit-reversed place between the passes; nothing is reordered in memory.  Inverse: the same steps backwards.
+//
+// k_fft_xy: one block per (y0, z); LX NY1 / 16 threads, 16 elements each; the tile lives in shared memory
+// (row stride LX + LX/8) between the row phase (x transform, T = LX/16 consecutive threads per row, exchanges
+// inside the row's warp) and the column phase (length-NY1 transform, lanes of a warp on adjacent columns).
+template <int RS> struct SmTileCol {
+    static constexpr bool TWPOW = true;
+    c2 *base; // already offset to this thread's column
+    __device__ __forceinline__ c2 &at(int n) { return base[n * RS]; }
+    __device__ __forceinline__ void sync() { __syncthreads(); }
+};
+
+template <int LX, int NY1, int DIR>
+__global__ void __launch_bounds__(LX *NY1 / 16, 1)
+    k_fft_xy(const c2 *__restrict__ in, c2 *__restrict__ out, const c2 *__restrict__ twx, const c2 *__restrict__ twy1, const c2 *__restrict__ twy,
+             int ny, int rev)
+{
+    constexpr int E = 16, TX = LX / E, RS = LX + LX / 8, T2 = NY1 / E;
+    static_assert(LX >= 64 && NY1 >= 16, "tile too small for 16 elements per thread");
+    extern __shared__ double2 smem[];
+    const int ny0 = ny / NY1;
+    const unsigned bid = rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const int y0 = bid % ny0;
+    const size_t z = bid / ny0;
+    const size_t tile0 = (z * ny + y0) * LX, rstride = (size_t)ny0 * LX; // row r of the tile starts at tile0 + r rstride
+    const int t = threadIdx.x;
+    const int r = t / TX, tid = t - r * TX;   // row phase
+    const int tid2 = t / LX, kx = t - tid2 * LX; // column phase
+    SmLine<TX> sl{smem + r * RS, 1 + r};
+    SmTileCol<RS> sc{smem + kx + (kx >> 3)};
+    c2 x[E];
+    if (DIR < 0) {
+        const c2 *row = in + tile0 + r * rstride;
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = row[tid + e * TX];
+        fft_line<LX, E, -1, 1, SmLine<TX>>(x, tid, twx, sl);
+#pragma unroll
+        for (int e = 0; e < E; ++e) sl.at(tid + e * TX) = x[e];
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = sc.at(tid2 + e * T2);
+        if (T2 > 1) __syncthreads(); // the exchanges of the column transform overwrite what its other threads read
+        fft_line<NY1, E, -1, 1, SmTileCol<RS>>(x, tid2, twy1, sc);
+        c2 *dst = out + tile0 + kx;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int ky1 = tid2 + e * T2;
+            dst[ky1 * rstride] = twmul<-1>(x[e], __ldg(&twy[(y0 * ky1) & (ny - 1)]));
+        }
+    } else {
+        const c2 *src = in + tile0 + kx;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int ky1 = tid2 + e * T2;
+            x[e] = twmul<+1>(src[ky1 * rstride], __ldg(&twy[(y0 * ky1) & (ny - 1)]));
+        }
+        fft_line<NY1, E, +1, 1, SmTileCol<RS>>(x, tid2, twy1, sc);
+#pragma unroll
+        for (int e = 0; e < E; ++e) sc.at(tid2 + e * T2) = x[e];
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = sl.at(tid + e * TX);
+        sl.sync();
+        fft_line<LX, E, +1, 1, SmLine<TX>>(x, tid, twx, sl);
+        c2 *row = out + tile0 + r * rstride;
+#pragma unroll
+        for (int e = 0; e < E; ++e) row[tid + e * TX] = x[e];
+    }
+}
+
+// k_fft_yz_solve: one block per (ky1, tile of XT adjacent kx): the NY0 LZ XT values (kx, y0, z) of the rows
+// ky1 NY0 + y0 -- forward transform over y0 (in registers: a thread first holds all NY0 values of 16/NY0 z planes),
+// forward over z, multiplication by inv_n / lambda, and both transforms backwards.  Shared-memory tile [z][ky0][kx].
+template <int N, int DIR> __device__ __forceinline__ void dft_small(c2 *v)
+{
+    if constexpr (N == 2) {
+        dft2<DIR>(v[0], v[1]);
+    } else if constexpr (N == 4) {
+        dft4<DIR>(v[0], v[1], v[2], v[3]);
+    } else if constexpr (N == 8) {
+        dft8<DIR>(*reinterpret_cast<c2(*)[8]>(v));
+    } else {
+        dft16<DIR>(*reinterpret_cast<c2(*)[16]>(v));
+    }
+}
+
+template <int STRIDE> struct SmStride {
+    static constexpr bool TWPOW = true;
+    c2 *base;
+    __device__ __forceinline__ c2 &at(int n) { return base[n * STRIDE]; }
+    __device__ __forceinline__ void sync() { __syncthreads(); }
+};
+
+template <int NY0, int LZ, int XT>
+__global__ void __launch_bounds__(XT *NY0 *LZ / 16)
+    k_fft_yz_solve(c2 *__restrict__ data, const c2 *__restrict__ twz, int mx, int ny, const double *__restrict__ ex, const double *__restrict__ ey,
+                   const double *__restrict__ ez, double inv_n, int rev)
+{
+    constexpr int E = 16, G = E / NY0, ZQ = LZ / G, T = LZ / E;
+    static_assert(NY0 >= 2 && NY0 <= 16 && LZ >= 32, "unsupported split");
+    extern __shared__ double2 smem[];
+    const int ny1 = ny / NY0, xtiles = mx / XT;
+    const unsigned bid = rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const int xt = bid % xtiles, ky1 = bid / xtiles;
+    const int t = threadIdx.x, xl = t % XT, rest = t / XT;
+    const int zq = rest;                          // first layout: all y0 of the planes zq + g ZQ
+    const int ky0 = rest % NY0, tid = rest / NY0; // second layout: planes tid + e T of one ky0
+    const size_t zstride = (size_t)mx * ny;
+    c2 *g1 = data + (size_t)ky1 * NY0 * mx + (size_t)xt * XT + xl;
+    c2 x[E];
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int y0 = 0; y0 < NY0; ++y0) x[g * NY0 + y0] = g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx];
+#pragma unroll
+    for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int q = 0; q < NY0; ++q) smem[((zq + g * ZQ) * NY0 + q) * XT + xl] = x[g * NY0 + q];
+    __syncthreads();
+    SmStride<NY0 * XT> sm{smem + ky0 * XT + xl};
+#pragma unroll
+    for (int e = 0; e < E; ++e) x[e] = sm.at(tid + e * T);
+    __syncthreads();
+    fft_line<LZ, E, -1, 1, SmStride<NY0 * XT>>(x, tid, twz, sm);
+    {
+        const int m = xt * XT + xl, ky = ky1 + ny1 * ky0;
+        const double exy = __ldg(&ex[m]) + __ldg(&ey[ky]);
+        const bool null_xy = (m == 0) && (((2 * ky) & (ny - 1)) == 0);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int kz = tid + e * T;
+            const double lam = -(exy + __ldg(&ez[kz]));
+            const bool null = null_xy && (((2 * kz) & (LZ - 1)) == 0);
+            const double sc = null ? 0.0 : inv_n * __drcp_rn(lam);
+            x[e].x = null ? 0.0 : x[e].x * sc;
+            x[e].y = null ? 0.0 : x[e].y * sc;
+        }
+    }
+    fft_line<LZ, E, +1, 1, SmStride<NY0 * XT>>(x, tid, twz, sm);
+#pragma unroll
+    for (int e = 0; e < E; ++e) sm.at(tid + e * T) = x[e];
+    __syncthreads();
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = smem[((zq + g * ZQ) * NY0 + q) * XT + xl];
+#pragma unroll
+    for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int y0 = 0; y0 < NY0; ++y0) g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx] = x[g * NY0 + y0];
+}
+
 } // namespace dnsfft

@@ -471,52 +471,62 @@ __global__ void __launch_bounds__(256) k_div(const double *__restrict__ u, const
 
 // a5, right-hand side of eq. 9: r = d + sum_a delta_a[(1-beta) delta_a p], evaluated only
 // where the bracket can be non-zero.  (1-beta) is 0 in the fluid, so those are the cells with at least
-// one solid face neighbour; `list` holds their linear indices in ascending order (built at create).
+// one solid face neighbour; `rec` holds one 64-bit record per such cell in ascending index order (built at
+// create): bits 0-31 the linear index, bits 32-38 the face byte, so that one coalesced load tells a thread
+// both where its cell is and which of the six p neighbours it needs -- every other load of the kernel can then
+// be issued at once (it was a chain of three dependent loads: index, face byte, neighbours).
 // The first iteration of a step saves d at those cells (`save`), later ones restore it from there, and
 // r overwrites d in place: everywhere else r == d already, so the forward x pass reads one plain array.
 // face: bit0 beta(cell), bit1/2 beta(x+1/x-1), bit3/4 beta(y+1/y-1), bit5/6 beta(z+1/z-1).
-constexpr int EQ9_ITEMS = 4; // list entries per thread: their loads are issued together (the kernel is a latency-bound gather)
+constexpr int EQ9_ITEMS = 4; // records per thread: their loads are issued together (the kernel is a latency-bound gather)
 template <bool FIRST>
-__global__ void __launch_bounds__(256) k_eq9_sparse(double *__restrict__ d, const double *__restrict__ p, const uint8_t *__restrict__ face,
-                                                    const uint32_t *__restrict__ list, double *__restrict__ save, int nlist, int nx, int ny,
-                                                    int nz, int lgx, int lgy, double r2x, double r2y, double r2z)
+__global__ void __launch_bounds__(256) k_eq9_sparse(double *__restrict__ d, const double *__restrict__ p, const unsigned long long *__restrict__ rec,
+                                                    double *__restrict__ save, int nlist, int nx, int ny, int nz, int lgx, int lgy,
+                                                    double r2x, double r2y, double r2z)
 {
     const int base = blockIdx.x * (256 * EQ9_ITEMS) + threadIdx.x;
-    uint32_t o[EQ9_ITEMS];
-    unsigned f[EQ9_ITEMS];
-    double dv[EQ9_ITEMS], pc[EQ9_ITEMS];
+    unsigned long long rc[EQ9_ITEMS];
 #pragma unroll
     for (int it = 0; it < EQ9_ITEMS; ++it) {
         const int n = base + it * 256;
-        o[it] = n < nlist ? __ldg(&list[n]) : 0u;
+        rc[it] = n < nlist ? __ldg(&rec[n]) : 0x7full << 32;
     }
+    double dv[EQ9_ITEMS], pc[EQ9_ITEMS], pn[EQ9_ITEMS][6];
 #pragma unroll
     for (int it = 0; it < EQ9_ITEMS; ++it) {
         const int n = base + it * 256;
-        f[it] = 0x7f;
+        const uint32_t oo = (uint32_t)rc[it];
+        const unsigned ff = (unsigned)(rc[it] >> 32);
+        const int i = oo & (nx - 1), j = (oo >> lgx) & (ny - 1), k = oo >> (lgx + lgy);
+        const size_t row = (size_t)nx * ((size_t)j + (size_t)ny * k);
         dv[it] = pc[it] = 0.0;
+#pragma unroll
+        for (int q = 0; q < 6; ++q) pn[it][q] = 0.0;
         if (n < nlist) {
-            f[it] = face[o[it]];
-            dv[it] = FIRST ? d[o[it]] : save[n];
-            pc[it] = __ldg(&p[o[it]]);
+            dv[it] = FIRST ? d[oo] : save[n];
+            pc[it] = __ldg(&p[oo]);
+            if (!(ff & 2)) pn[it][0] = __ldg(&p[row + ((i + 2) & (nx - 1))]);
+            if (!(ff & 4)) pn[it][1] = __ldg(&p[row + ((i - 2) & (nx - 1))]);
+            if (!(ff & 8)) pn[it][2] = __ldg(&p[(size_t)nx * ((size_t)((j + 2) & (ny - 1)) + (size_t)ny * k) + i]);
+            if (!(ff & 16)) pn[it][3] = __ldg(&p[(size_t)nx * ((size_t)((j - 2) & (ny - 1)) + (size_t)ny * k) + i]);
+            if (!(ff & 32)) pn[it][4] = __ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k + 2) & (nz - 1))) + i]);
+            if (!(ff & 64)) pn[it][5] = __ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k - 2) & (nz - 1))) + i]);
         }
     }
 #pragma unroll
     for (int it = 0; it < EQ9_ITEMS; ++it) {
         const int n = base + it * 256;
         if (n >= nlist) continue;
-        const uint32_t oo = o[it];
-        const unsigned ff = f[it];
-        const int i = oo & (nx - 1), j = (oo >> lgx) & (ny - 1), k = oo >> (lgx + lgy);
+        const uint32_t oo = (uint32_t)rc[it];
+        const unsigned ff = (unsigned)(rc[it] >> 32);
         if (FIRST) save[n] = dv[it];
-        const size_t row = (size_t)nx * ((size_t)j + (size_t)ny * k);
         double gxp = 0.0, gxm = 0.0, gyp = 0.0, gym = 0.0, gzp = 0.0, gzm = 0.0;
-        if (!(ff & 2)) gxp = (__ldg(&p[row + ((i + 2) & (nx - 1))]) - pc[it]) * r2x;
-        if (!(ff & 4)) gxm = (pc[it] - __ldg(&p[row + ((i - 2) & (nx - 1))])) * r2x;
-        if (!(ff & 8)) gyp = (__ldg(&p[(size_t)nx * ((size_t)((j + 2) & (ny - 1)) + (size_t)ny * k) + i]) - pc[it]) * r2y;
-        if (!(ff & 16)) gym = (pc[it] - __ldg(&p[(size_t)nx * ((size_t)((j - 2) & (ny - 1)) + (size_t)ny * k) + i])) * r2y;
-        if (!(ff & 32)) gzp = (__ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k + 2) & (nz - 1))) + i]) - pc[it]) * r2z;
-        if (!(ff & 64)) gzm = (pc[it] - __ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k - 2) & (nz - 1))) + i])) * r2z;
+        if (!(ff & 2)) gxp = (pn[it][0] - pc[it]) * r2x;
+        if (!(ff & 4)) gxm = (pc[it] - pn[it][1]) * r2x;
+        if (!(ff & 8)) gyp = (pn[it][2] - pc[it]) * r2y;
+        if (!(ff & 16)) gym = (pc[it] - pn[it][3]) * r2y;
+        if (!(ff & 32)) gzp = (pn[it][4] - pc[it]) * r2z;
+        if (!(ff & 64)) gzm = (pc[it] - pn[it][5]) * r2z;
         d[oo] = dv[it] + ((gxp - gxm) * r2x + (gyp - gym) * r2y + (gzp - gzm) * r2z);
     }
 }
