@@ -230,10 +230,10 @@ void dnsref_fft1d(int n, double *re, double *im, int sign)
     }
     for (int len = 2; len <= n; len <<= 1) {
         int half = len >> 1;
-        for (int s = 0; s < n; s += len)
-            for (int j = 0; j < half; ++j) {
-                double a = sign * 2.0 * M_PI * (double)j / len;
-                double wr = cos(a), wi = sin(a);
+        for (int j = 0; j < half; ++j) { /* twiddle j of this level, then its butterfly in every block of the level */
+            double a = sign * 2.0 * M_PI * (double)j / len;
+            double wr = cos(a), wi = sin(a);
+            for (int s = 0; s < n; s += len) {
                 double xr = re[s + j + half] * wr - im[s + j + half] * wi;
                 double xi = re[s + j + half] * wi + im[s + j + half] * wr;
                 re[s + j + half] = re[s + j] - xr;
@@ -241,6 +241,7 @@ void dnsref_fft1d(int n, double *re, double *im, int sign)
                 re[s + j] += xr;
                 im[s + j] += xi;
             }
+        }
     }
 }
 
@@ -292,6 +293,7 @@ int dnsref_poisson_solve(dnsref_t *h, const double *r, double *p)
     const int nx = h->P.nx, ny = h->P.ny, nz = h->P.nz;
     const int64_t n = h->n;
     double *re = h->re, *im = h->im;
+#pragma omp parallel for schedule(static)
     for (int64_t o = 0; o < n; ++o) { re[o] = r[o]; im[o] = 0.0; }
     dnsref_fft3(nx, ny, nz, re, im, -1);
 #pragma omp parallel for schedule(static)
@@ -308,6 +310,7 @@ int dnsref_poisson_solve(dnsref_t *h, const double *r, double *p)
                 }
             }
     dnsref_fft3(nx, ny, nz, re, im, +1);
+#pragma omp parallel for schedule(static)
     for (int64_t o = 0; o < n; ++o) p[o] = re[o] / (double)n;
     return DNSREF_OK;
 }
@@ -426,11 +429,13 @@ int dnsref_step(dnsref_t *h, int nsteps)
         }
         for (int s = 0; s < 4; ++s) {
             dnsref_rhs(h, h->qs[0], h->qs[1], h->qs[2], h->qs[3], h->f[0], h->f[1], h->f[2], h->f[3]);
-            for (int m = 0; m < 4; ++m)
+            for (int m = 0; m < 4; ++m) {
+#pragma omp parallel for schedule(static)
                 for (int64_t o = 0; o < n; ++o) {
                     h->qc[m][o] = h->qc[m][o] + (b[s] * dt) * h->f[m][o];
                     if (s < 3) h->qs[m][o] = h->q[m][o] + (a[s] * dt) * h->f[m][o];
                 }
+            }
             if (s < 3 && (h->P.flags & 2u)) {
                 /* NEXT-2 variant: project the stage velocity, using a scratch pressure */
                 double *ps = (double *)malloc(sizeof(double) * n);
