@@ -47,6 +47,8 @@ def class_bytes_per_cell(masked, fb=0.0):
         "fft_x": 16.0,
         "fft_y": 16.0,
         "fft_z_solve": 16.0,
+        "fft_xy": 16.0,         # two-pass solve: x and the high digit of y (R1 W1 of the complex array, 8 B/cell each way)
+        "fft_yz_solve": 16.0,   # two-pass solve: low digit of y, z, division, and back (R1 W1)
         "project": 56.0 + m,
         "eq9_sparse": 8.0 + m,
         "filter": 64.0 + m,
@@ -325,9 +327,9 @@ def run_ours(args):
     peak, peak_src = load_peak()
     achieved = cb[dom] * N / (d_ms / d_n * 1e-3) / 1e9
     achieved_moved = mv[dom] * N / (d_ms / d_n * 1e-3) / 1e9
-    breakdown = {k: {"ms_per_step": v[0] / K, "launches_per_step": v[1] / K,
-                     "GBps_canonical": cb[k] * N / (v[0] / v[1] * 1e-3) / 1e9,
-                     "GBps_moved": mv[k] * N / (v[0] / v[1] * 1e-3) / 1e9} for k, v in prof.items()}
+    breakdown = {k: {"ms_per_step": v[0] / K, "launches_per_step": v[1] / K, "us_per_launch": v[0] / v[1] * 1e3,
+                     "GBps_canonical": cb.get(k, 0.0) * N / (v[0] / v[1] * 1e-3) / 1e9,
+                     "GBps_moved": mv.get(k, 0.0) * N / (v[0] / v[1] * 1e-3) / 1e9} for k, v in prof.items()}
     traffic, traffic_src = ncu_traffic(args.traffic_csv, dom, case)
     step_bytes = (canonical_bytes_per_cell(P, masked) + (cb["filter"] if args.flags & 1 else 0.0)) * N
     step_gbs = step_bytes / (ms_max / K * 1e-3) / 1e9

@@ -122,7 +122,8 @@ struct dnslab {
     dim3 rk_block;
     int nsm;   // SM count of the device
     bool prepare; // set while dnslab_create walks the launchers once: they configure their kernel and do not launch
-    unsigned zgrid; // grid of the persistent fused z pass (occupancy query done once, at create)
+    unsigned zgrid; // grid of the persistent fused middle pass (occupancy query done once, at create)
+    int xy_ahead; // two-pass solve, xy passes: how many blocks ahead a block prefetches into L2 (blocks resident on the chip)
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
     long long np;      // NEXT-4: attached particles (0: none); state is the caller's device array
     double *pstate, prho_f, pgrav[3];
@@ -389,31 +390,44 @@ int launch_fft_z_solve(dnslab *h, c2 *data)
 // A tile of the xy pass is 8192 complex numbers (NY1 = 8192 / (nx/2) whole rows, 144 KB of shared memory with padding);
 // the fused middle pass takes NY0 = ny / NY1 rows by all of z for XT adjacent kx, at most 8192 numbers again.
 // Shapes outside these limits (and masks that need the dense eq. 9 prologue) use the five single-axis passes.
-constexpr int XY_TILE = 8192;
+#ifndef DNSLAB_XY_TILE
+#define DNSLAB_XY_TILE 4096
+#endif
+#ifndef DNSLAB_YZ_TILE
+#define DNSLAB_YZ_TILE 8192
+#endif
+#ifndef DNSLAB_YZ_XTMIN
+#define DNSLAB_YZ_XTMIN 4
+#endif
+constexpr int XY_TILE = DNSLAB_XY_TILE, YZ_TILE = DNSLAB_YZ_TILE, YZ_XTMIN = DNSLAB_YZ_XTMIN;
+constexpr int xy_rows(int mx) { return XY_TILE / mx < 16 ? 16 : XY_TILE / mx; } // rows of an xy tile: at least 16 (one radix-16 column butterfly)
 
 int fused_ny1(const dnslab_params_t *P)
 {
     const int mx = P->nx / 2;
     if (mx < 64 || mx > 512) return 0;
-    const int ny1 = XY_TILE / mx; // 128, 64, 32, 16
+    const int ny1 = xy_rows(mx);
     if (P->ny < ny1) return 0;
     const int ny0 = P->ny / ny1;
     if (ny0 == 1) return ny1; // the middle pass is then the plain fused z pass
-    if (ny0 > 16 || P->nz < 32 || ny0 * P->nz > 2048) return 0;
+    if (ny0 > 16 || P->nz < 32 || ny0 * P->nz * YZ_XTMIN > YZ_TILE) return 0;
     return ny1;
 }
 
 template <int LX, int DIR> int launch_fft_xy_L(dnslab *h, const c2 *in, c2 *out)
 {
-    constexpr int NY1 = XY_TILE / LX, NT = XY_TILE / 16;
+    constexpr int NY1 = xy_rows(LX), NT = LX * NY1 / 16;
     const size_t smem = (size_t)NY1 * (LX + LX / 8) * sizeof(c2);
     auto kern = dnsfft::k_fft_xy<LX, NY1, DIR>;
     if (h->prepare) {
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int per_sm = 0;
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
+        h->xy_ahead = per_sm * h->nsm; // the block that takes over an SM when this one retires
         return DNSLAB_OK;
     }
     ProfScope ps(h, DNSLAB_K_FFT_XY);
-    kern<<<(unsigned)((h->P.ny / NY1) * h->P.nz), NT, smem, h->stream>>>(in, out, h->tw[0], h->twy1, h->tw[1], h->P.ny, DIR < 0 ? 0 : 1);
+    kern<<<(unsigned)((h->P.ny / NY1) * h->P.nz), NT, smem, h->stream>>>(in, out, h->tw[0], h->twy1, h->tw[1], h->P.ny, DIR < 0 ? 0 : 1, h->xy_ahead);
     return check_launch(h);
 }
 
@@ -430,17 +444,14 @@ template <int DIR> int launch_fft_xy(dnslab *h, const c2 *in, c2 *out)
 
 template <int NY0, int LZ> int launch_fft_yz_solve_NL(dnslab *h, c2 *data)
 {
-    constexpr int XT = (XY_TILE / (NY0 * LZ)) > 16 ? 16 : XY_TILE / (NY0 * LZ), NT = XT * NY0 * LZ / 16;
-    const size_t smem = (size_t)XT * NY0 * LZ * sizeof(c2);
-    auto kern = dnsfft::k_fft_yz_solve<NY0, LZ, XT>;
-    if (h->prepare) {
-        if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        return DNSLAB_OK;
-    }
+    constexpr int XT = (YZ_TILE / (NY0 * LZ)) > 16 ? 16 : ((YZ_TILE / (NY0 * LZ)) < 1 ? 1 : YZ_TILE / (NY0 * LZ)), NT = XT * NY0 * LZ / 16;
+    const size_t smem = (size_t)LZ * (NY0 * XT + (XT < 8 ? XT : 0)) * sizeof(c2) + LZ * sizeof(double);
     const int mx = h->P.nx / 2;
+    const size_t ntiles = (size_t)(mx / XT) * (h->P.ny / NY0);
+    auto kern = dnsfft::k_fft_yz_solve<NY0, LZ, XT>;
+    if (h->prepare) return persistent_grid(h, kern, NT, smem, ntiles, &h->zgrid);
     ProfScope ps(h, DNSLAB_K_FFT_YZ);
-    kern<<<(unsigned)((mx / XT) * (h->P.ny / NY0)), NT, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2],
-                                                                          2.0 / (double)h->n, 1);
+    kern<<<h->zgrid, NT, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], 2.0 / (double)h->n, (int)ntiles, 1);
     return check_launch(h);
 }
 

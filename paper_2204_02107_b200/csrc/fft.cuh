@@ -265,6 +265,16 @@ __device__ __forceinline__ void cp_async_c2(c2 *dst_smem, const c2 *src)
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
+// Ask L2 for `bytes` (multiple of 16) starting at the 16-byte aligned global address p; no register, no wait.
+// The two-pass kernels hold one tile per SM in shared memory, so a block cannot stage its successor's tile on chip;
+// it asks for it in L2 instead, while it computes (the blocks of a grid are handed out in index order).
+__device__ __forceinline__ void prefetch_l2(const void *p, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(p), "r"(bytes) : "memory");
+}
+// The same for one cache line, as an ordinary per-lane instruction (the bulk form runs on the uniform datapath: a
+// warp whose lanes hold different addresses executes it once per lane, 25 instructions per element in k_fft_yz_solve)
+__device__ __forceinline__ void prefetch_l2_line(const void *p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p) : "memory"); }
 
 // x pass: lines of L = nx/2 complex numbers, contiguous.  NL lines per block, one line per T consecutive
 // threads, so the exchanges of a line never leave its warp (or its named barrier).
@@ -330,6 +340,18 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 
     for (int e = 0; e < E; ++e) base[(size_t)(tid + e * T) * stride] = x[e];
 }
 
+// 1/a for finite, normal a != 0: hardware seed (rcp.approx, 20 bits) and two Newton steps -- about an ulp, no special
+// cases, a third of the instructions of a correctly rounded reciprocal.  lambda is bounded away from 0 and from
+// overflow on every non-null mode; null modes are replaced by 0 by the caller.
+__device__ __forceinline__ double rcp_newton(double a)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+    r = fma(r, fma(-a, r, 1.0), r);
+    r = fma(r, fma(-a, r, 1.0), r);
+    return r;
+}
+
 // Fused middle pass along z: forward transform, division by the modified-wavenumber eigenvalue
 //   lambda(m,ky,kz) = -(ex[m] + ey[ky] + ez[kz]),  e_a[k] = (sin(2 pi k/N_a)/D_a)^2,
 // null modes (m = 0, 2ky = 0 mod ny, 2kz = 0 mod nz) set to 0, scaling by 1/N, inverse transform.
@@ -378,7 +400,7 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 
             const int kz = tid + e * T;
             const double lam = -(exy + ezr[e]);
             const bool null = null_xy && (((2 * kz) & (L - 1)) == 0);
-            const double s = null ? 0.0 : inv_n * __drcp_rn(lam); // reciprocal + product: a third of a full division's instructions
+            const double s = inv_n * rcp_newton(lam);
             x[e].x = null ? 0.0 : x[e].x * s;
             x[e].y = null ? 0.0 : x[e].y * s;
         }
@@ -410,9 +432,9 @@ template <int RS> struct SmTileCol {
 };
 
 template <int LX, int NY1, int DIR>
-__global__ void __launch_bounds__(LX *NY1 / 16, 1)
+__global__ void __launch_bounds__(LX *NY1 / 16, (LX * NY1 / 16 <= 256 ? 2 : 1))
     k_fft_xy(const c2 *__restrict__ in, c2 *__restrict__ out, const c2 *__restrict__ twx, const c2 *__restrict__ twy1, const c2 *__restrict__ twy,
-             int ny, int rev)
+             int ny, int rev, int ahead)
 {
     constexpr int E = 16, TX = LX / E, RS = LX + LX / 8, T2 = NY1 / E;
     static_assert(LX >= 64 && NY1 >= 16, "tile too small for 16 elements per thread");
@@ -423,15 +445,26 @@ __global__ void __launch_bounds__(LX *NY1 / 16, 1)
     const size_t z = bid / ny0;
     const size_t tile0 = (z * ny + y0) * LX, rstride = (size_t)ny0 * LX; // row r of the tile starts at tile0 + r rstride
     const int t = threadIdx.x;
-    const int r = t / TX, tid = t - r * TX;   // row phase
+    const int r = t / TX, tid = t - r * TX;      // row phase
     const int tid2 = t / LX, kx = t - tid2 * LX; // column phase
     SmLine<TX> sl{smem + r * RS, 1 + r};
     SmTileCol<RS> sc{smem + kx + (kx >> 3)};
     c2 x[E];
+    // One block per tile (a persistent block walking several tiles measured slower here: 58 against 52 us per pass on
+    // 512x256x128).  While it computes, the block asks L2 for the tile of the block `ahead` places behind it in launch
+    // order -- the one that will take over an SM about when this one retires -- one row per thread.
+    auto prefetch_next = [&]() {
+        const unsigned nb = blockIdx.x + ahead;
+        if (ahead > 0 && nb < gridDim.x && t < NY1) {
+            const unsigned nbid = rev ? gridDim.x - 1 - nb : nb;
+            prefetch_l2(in + ((size_t)(nbid / ny0) * ny + nbid % ny0) * LX + t * rstride, LX * sizeof(c2));
+        }
+    };
     if (DIR < 0) {
         const c2 *row = in + tile0 + r * rstride;
 #pragma unroll
         for (int e = 0; e < E; ++e) x[e] = row[tid + e * TX];
+        prefetch_next();
         fft_line<LX, E, -1, 1, SmLine<TX>>(x, tid, twx, sl);
 #pragma unroll
         for (int e = 0; e < E; ++e) sl.at(tid + e * TX) = x[e];
@@ -453,6 +486,7 @@ __global__ void __launch_bounds__(LX *NY1 / 16, 1)
             const int ky1 = tid2 + e * T2;
             x[e] = twmul<+1>(src[ky1 * rstride], __ldg(&twy[(y0 * ky1) & (ny - 1)]));
         }
+        prefetch_next();
         fft_line<NY1, E, +1, 1, SmTileCol<RS>>(x, tid2, twy1, sc);
 #pragma unroll
         for (int e = 0; e < E; ++e) sc.at(tid2 + e * T2) = x[e];
@@ -491,66 +525,86 @@ template <int STRIDE> struct SmStride {
 };
 
 template <int NY0, int LZ, int XT>
-__global__ void __launch_bounds__(XT *NY0 *LZ / 16)
+__global__ void __launch_bounds__(XT *NY0 *LZ / 16, (XT * NY0 * LZ / 16 <= 256 ? 2 : 1))
     k_fft_yz_solve(c2 *__restrict__ data, const c2 *__restrict__ twz, int mx, int ny, const double *__restrict__ ex, const double *__restrict__ ey,
-                   const double *__restrict__ ez, double inv_n, int rev)
+                   const double *__restrict__ ez, double inv_n, int ntiles, int rev)
 {
-    constexpr int E = 16, G = E / NY0, ZQ = LZ / G, T = LZ / E;
+    constexpr int E = 16, G = E / NY0, ZQ = LZ / G, T = LZ / E, NT = XT * NY0 * LZ / E;
+    // one z plane of the tile: NY0 XT numbers, padded so that the quarter-warps of both layouts hit 32 different banks
+    constexpr int ZROW = NY0 * XT + (XT < 8 ? XT : 0);
     static_assert(NY0 >= 2 && NY0 <= 16 && LZ >= 32, "unsupported split");
     extern __shared__ double2 smem[];
+    double *sez = reinterpret_cast<double *>(smem + LZ * ZROW); // the z eigenvalue parts, read LZ times per tile
     const int ny1 = ny / NY0, xtiles = mx / XT;
-    const unsigned bid = rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
-    const int xt = bid % xtiles, ky1 = bid / xtiles;
     const int t = threadIdx.x, xl = t % XT, rest = t / XT;
     const int zq = rest;                          // first layout: all y0 of the planes zq + g ZQ
     const int ky0 = rest % NY0, tid = rest / NY0; // second layout: planes tid + e T of one ky0
     const size_t zstride = (size_t)mx * ny;
-    c2 *g1 = data + (size_t)ky1 * NY0 * mx + (size_t)xt * XT + xl;
-    c2 x[E];
+    for (int q = t; q < LZ; q += NT) sez[q] = ez[q];
+    for (int lt = blockIdx.x; lt < ntiles; lt += gridDim.x) {
+        const unsigned bid = rev ? ntiles - 1 - lt : lt;
+        const int xt = bid % xtiles, ky1 = bid / xtiles;
+        c2 *g1 = data + (size_t)ky1 * NY0 * mx + (size_t)xt * XT + xl;
+        c2 x[E];
 #pragma unroll
-    for (int g = 0; g < G; ++g)
+        for (int g = 0; g < G; ++g)
 #pragma unroll
-        for (int y0 = 0; y0 < NY0; ++y0) x[g * NY0 + y0] = g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx];
-#pragma unroll
-    for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
-#pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int q = 0; q < NY0; ++q) smem[((zq + g * ZQ) * NY0 + q) * XT + xl] = x[g * NY0 + q];
-    __syncthreads();
-    SmStride<NY0 * XT> sm{smem + ky0 * XT + xl};
-#pragma unroll
-    for (int e = 0; e < E; ++e) x[e] = sm.at(tid + e * T);
-    __syncthreads();
-    fft_line<LZ, E, -1, 1, SmStride<NY0 * XT>>(x, tid, twz, sm);
-    {
+            for (int y0 = 0; y0 < NY0; ++y0) x[g * NY0 + y0] = g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx];
         const int m = xt * XT + xl, ky = ky1 + ny1 * ky0;
         const double exy = __ldg(&ex[m]) + __ldg(&ey[ky]);
-        const bool null_xy = (m == 0) && (((2 * ky) & (ny - 1)) == 0);
+        if (lt + (int)gridDim.x < ntiles) {
+            // this block's next tile into L2 while this one is computed: LZ NY0 runs of XT complex numbers,
+            // one request per 128 bytes of each run
+            const unsigned nbid = rev ? ntiles - 1 - (lt + gridDim.x) : lt + gridDim.x;
+            const c2 *nt = data + (size_t)(nbid / xtiles) * NY0 * mx + (size_t)(nbid % xtiles) * XT;
+            constexpr int PER_RUN = XT >= 8 ? XT / 8 : 1, RUNS = LZ * NY0, REQ = RUNS * PER_RUN;
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-            const int kz = tid + e * T;
-            const double lam = -(exy + __ldg(&ez[kz]));
-            const bool null = null_xy && (((2 * kz) & (LZ - 1)) == 0);
-            const double sc = null ? 0.0 : inv_n * __drcp_rn(lam);
-            x[e].x = null ? 0.0 : x[e].x * sc;
-            x[e].y = null ? 0.0 : x[e].y * sc;
+            for (int q0 = 0; q0 < (REQ + NT - 1) / NT; ++q0) {
+                const int q = t + q0 * NT, run = q / PER_RUN, part = q % PER_RUN; // (z, y0) = (run / NY0, run % NY0)
+                if (q < REQ) prefetch_l2_line(nt + (size_t)(run / NY0) * zstride + (size_t)(run % NY0) * mx + part * 8);
+            }
         }
+#pragma unroll
+        for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int q = 0; q < NY0; ++q) smem[(zq + g * ZQ) * ZROW + q * XT + xl] = x[g * NY0 + q];
+        __syncthreads();
+        SmStride<ZROW> sm{smem + ky0 * XT + xl};
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = sm.at(tid + e * T);
+        __syncthreads();
+        fft_line<LZ, E, -1, 1, SmStride<ZROW>>(x, tid, twz, sm);
+        {
+            const bool null_xy = (m == 0) && (((2 * ky) & (ny - 1)) == 0);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int kz = tid + e * T;
+                const double lam = -(exy + sez[kz]);
+                const bool null = null_xy && (((2 * kz) & (LZ - 1)) == 0);
+                const double sc = inv_n * rcp_newton(lam);
+                x[e].x = null ? 0.0 : x[e].x * sc;
+                x[e].y = null ? 0.0 : x[e].y * sc;
+            }
+        }
+        fft_line<LZ, E, +1, 1, SmStride<ZROW>>(x, tid, twz, sm);
+#pragma unroll
+        for (int e = 0; e < E; ++e) sm.at(tid + e * T) = x[e];
+        __syncthreads();
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = smem[(zq + g * ZQ) * ZROW + q * XT + xl];
+#pragma unroll
+        for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int y0 = 0; y0 < NY0; ++y0) g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx] = x[g * NY0 + y0];
+        // the first layout's slots are private to a thread (it reads back exactly what it wrote), so the next
+        // tile may start without another barrier
     }
-    fft_line<LZ, E, +1, 1, SmStride<NY0 * XT>>(x, tid, twz, sm);
-#pragma unroll
-    for (int e = 0; e < E; ++e) sm.at(tid + e * T) = x[e];
-    __syncthreads();
-#pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = smem[((zq + g * ZQ) * NY0 + q) * XT + xl];
-#pragma unroll
-    for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
-#pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int y0 = 0; y0 < NY0; ++y0) g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx] = x[g * NY0 + y0];
 }
 
 } // namespace dnsfft

@@ -478,7 +478,7 @@ __global__ void __launch_bounds__(256) k_div(const double *__restrict__ u, const
 // The first iteration of a step saves d at those cells (`save`), later ones restore it from there, and
 // r overwrites d in place: everywhere else r == d already, so the forward x pass reads one plain array.
 // face: bit0 beta(cell), bit1/2 beta(x+1/x-1), bit3/4 beta(y+1/y-1), bit5/6 beta(z+1/z-1).
-constexpr int EQ9_ITEMS = 4; // records per thread: their loads are issued together (the kernel is a latency-bound gather)
+constexpr int EQ9_ITEMS = 1; // records per thread (4 with all loads issued together needs ~100 registers and measured slower: occupancy matters more here)
 template <bool FIRST>
 __global__ void __launch_bounds__(256) k_eq9_sparse(double *__restrict__ d, const double *__restrict__ p, const unsigned long long *__restrict__ rec,
                                                     double *__restrict__ save, int nlist, int nx, int ny, int nz, int lgx, int lgy,

@@ -65,13 +65,14 @@ def test_poisson_matches_oracle(shape):
 
 
 # Shapes that take the two-pass solve (k_fft_xy + k_fft_yz_solve): every xy tile shape
-# (nx = 128, 256, 512, 1024) and every (NY0, nz) instantiation of the fused middle pass, plus NY0 = 1 (plain z pass).
-@pytest.mark.parametrize("shape", [(32, 128, 128), (32, 256, 128), (64, 64, 256), (32, 256, 256), (64, 128, 256),
-                                   (128, 256, 512), (32, 32, 512), (64, 512, 512), (32, 16, 1024), (32, 256, 1024),
-                                   (128, 128, 1024), (256, 256, 256), (512, 128, 256), (1024, 128, 256), (512, 256, 256),
-                                   (256, 256, 512), (128, 1024, 128), (128, 128, 256), (256, 128, 256), (128, 512, 512), (64, 1024, 128),
-                                   (32, 1024, 128), (32, 512, 128), (128, 512, 128), (256, 512, 128), (64, 256, 256),
-                                   (32, 128, 256), (32, 512, 512), (32, 128, 1024), (64, 128, 1024), (64, 256, 1024)])
+# (nx = 128, 256, 512, 1024), every (NY0, nz) instantiation of the fused middle pass (NY0 = ny / rows of an xy tile in
+# {2, 4, 8, 16}, NY0 nz <= 2048), NY0 = 1 (plain fused z pass in the middle), and the grids of configs 3 and 4.
+@pytest.mark.parametrize("shape", [(32, 128, 128), (64, 128, 128), (128, 128, 128), (256, 128, 128), (512, 128, 128),
+                                   (1024, 128, 128), (32, 256, 128), (64, 256, 128), (128, 256, 128), (256, 256, 128),
+                                   (512, 256, 128), (32, 512, 128), (64, 512, 128), (128, 512, 128), (256, 512, 128),
+                                   (32, 1024, 128), (64, 1024, 128), (128, 1024, 128), (32, 64, 128), (32, 32, 256),
+                                   (64, 16, 512), (32, 16, 1024), (128, 256, 512), (256, 256, 256), (64, 256, 1024),
+                                   (128, 128, 1024)])
 def test_poisson_two_pass_shapes_match_oracle(shape):
     import torch
     rng = np.random.default_rng(sum(shape) + 1)
