@@ -123,6 +123,7 @@ struct dnslab {
     int nsm;   // SM count of the device
     bool prepare; // set while dnslab_create walks the launchers once: they configure their kernel and do not launch
     unsigned zgrid; // grid of the persistent fused middle pass (occupancy query done once, at create)
+    int yz_ahead; // the same for the fused middle pass
     int xy_ahead; // two-pass solve, xy passes: how many blocks ahead a block prefetches into L2 (blocks resident on the chip)
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
     long long np;      // NEXT-4: attached particles (0: none); state is the caller's device array
@@ -417,7 +418,7 @@ int fused_ny1(const dnslab_params_t *P)
 template <int LX, int DIR> int launch_fft_xy_L(dnslab *h, const c2 *in, c2 *out)
 {
     constexpr int NY1 = xy_rows(LX), NT = LX * NY1 / 16;
-    const size_t smem = (size_t)NY1 * (LX + LX / 8) * sizeof(c2);
+    const size_t smem = (size_t)NY1 * (LX + LX / 16) * sizeof(c2);
     auto kern = dnsfft::k_fft_xy<LX, NY1, DIR>;
     if (h->prepare) {
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -445,13 +446,19 @@ template <int DIR> int launch_fft_xy(dnslab *h, const c2 *in, c2 *out)
 template <int NY0, int LZ> int launch_fft_yz_solve_NL(dnslab *h, c2 *data)
 {
     constexpr int XT = (YZ_TILE / (NY0 * LZ)) > 16 ? 16 : ((YZ_TILE / (NY0 * LZ)) < 1 ? 1 : YZ_TILE / (NY0 * LZ)), NT = XT * NY0 * LZ / 16;
-    const size_t smem = (size_t)LZ * (NY0 * XT + (XT < 8 ? XT : 0)) * sizeof(c2) + LZ * sizeof(double);
+    const size_t smem = (size_t)LZ * (NY0 * XT + (XT < 8 ? XT : 0)) * sizeof(c2) + LZ * (sizeof(c2) + sizeof(double));
     const int mx = h->P.nx / 2;
-    const size_t ntiles = (size_t)(mx / XT) * (h->P.ny / NY0);
     auto kern = dnsfft::k_fft_yz_solve<NY0, LZ, XT>;
-    if (h->prepare) return persistent_grid(h, kern, NT, smem, ntiles, &h->zgrid);
+    if (h->prepare) {
+        if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int per_sm = 0;
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
+        h->yz_ahead = per_sm * h->nsm;
+        return DNSLAB_OK;
+    }
     ProfScope ps(h, DNSLAB_K_FFT_YZ);
-    kern<<<h->zgrid, NT, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], 2.0 / (double)h->n, (int)ntiles, 1);
+    kern<<<(unsigned)((mx / XT) * (h->P.ny / NY0)), NT, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2],
+                                                                          2.0 / (double)h->n, 1, h->yz_ahead);
     return check_launch(h);
 }
 

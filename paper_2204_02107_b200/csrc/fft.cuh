@@ -113,7 +113,7 @@ template <int DIR> __device__ __forceinline__ void dft16(c2 (&v)[16])
 // One Stockham stage of radix R on the E register elements of thread `tid` (element e <-> index
 // tid + e*T).  Ns = product of the radices of the earlier stages.  On exit slot q + r*(E/R) holds
 // output r of butterfly jj = tid + q*T, whose natural position is oidx = expand(jj) + r*Ns.
-template <int L, int E, int R, int NS, int DIR, bool TWPOW> __device__ __forceinline__ void stage(c2 (&x)[E], int tid, const c2 *__restrict__ tw)
+template <int L, int E, int R, int NS, int DIR, bool TWPOW, bool TWSMEM = false> __device__ __forceinline__ void stage(c2 (&x)[E], int tid, const c2 *__restrict__ tw)
 {
     constexpr int T = L / E;
     constexpr int Q = E / R;
@@ -147,7 +147,7 @@ template <int L, int E, int R, int NS, int DIR, bool TWPOW> __device__ __forcein
                 for (int r = 1; r < R; ++r) v[r] = twmul<DIR>(v[r], w[r]);
             } else {
 #pragma unroll
-                for (int r = 1; r < R; ++r) v[r] = twmul<DIR>(v[r], __ldg(&tw[kb * r]));
+                for (int r = 1; r < R; ++r) v[r] = twmul<DIR>(v[r], TWSMEM ? tw[kb * r] : __ldg(&tw[kb * r]));
             }
         }
         if constexpr (R == 16) {
@@ -164,6 +164,11 @@ template <int L, int E, int R, int NS, int DIR, bool TWPOW> __device__ __forcein
     }
 }
 
+// a view may declare `static constexpr bool TWSMEM = true`: the twiddle table passed to fft_line then lives in shared
+// memory and is read with plain loads, one look-up per twiddle (lanes that share a butterfly index broadcast)
+template <class SM, class = void> struct tw_in_smem { static constexpr bool value = false; };
+template <class SM> struct tw_in_smem<SM, decltype((void)SM::TWSMEM)> { static constexpr bool value = SM::TWSMEM; };
+
 template <int L, int E, int NS> struct NextRadix {
     static constexpr int rem = L / NS;
     static constexpr int cap = E >= 16 ? 16 : (E >= 8 ? 8 : E);
@@ -178,7 +183,7 @@ template <int L, int E, int DIR, int NS, class SM> __device__ __forceinline__ vo
     constexpr int T = L / E;
     constexpr int R = NextRadix<L, E, NS>::value;
     constexpr int Q = E / R;
-    stage<L, E, R, NS, DIR, SM::TWPOW>(x, tid, tw);
+    stage<L, E, R, NS, DIR, SM::TWPOW, tw_in_smem<SM>::value>(x, tid, tw);
     if constexpr (NS * R < L) {
 #pragma unroll
         for (int q = 0; q < Q; ++q) {
@@ -200,11 +205,14 @@ template <int L, int E, int DIR, int NS, class SM> __device__ __forceinline__ vo
 // contiguous line with one pad element per 8 (x pass: threads of a warp walk along the line)
 // The T threads of a line are T consecutive threads: inside one warp for T <= 32 (__syncwarp), else a
 // named barrier per line (id 1 + line-in-block, at most 15 lines per block then).
-template <int T> struct SmLine {
+// PSH: one pad element per 2^PSH.  A thread writes runs of R consecutive elements after a radix-R stage, so the lanes
+// of a quarter-warp are R elements apart: with R = 16 the pad must come every 16 (stride 17 = 1 mod 8 sixteen-byte
+// units, conflict-free); every 8 leaves a two-way conflict there (measured: 23 % of the wavefronts of k_fft_xy).
+template <int T, int PSH = 3> struct SmLine {
     static constexpr bool TWPOW = true;
     c2 *base;
     int bar;
-    __device__ __forceinline__ c2 &at(int n) { return base[n + (n >> 3)]; }
+    __device__ __forceinline__ c2 &at(int n) { return base[n + (n >> PSH)]; }
     __device__ __forceinline__ void sync()
     {
         if constexpr (T <= 32) __syncwarp();
@@ -422,7 +430,7 @@ __global__ void __launch_bounds__(XT *(L / ElemsPerThreadZ<L>::value) < 32 ? 32 
 // digit-reversed place between the passes; nothing is reordered in memory.  Inverse: the same steps backwards.
 //
 // k_fft_xy: one block per (y0, z); LX NY1 / 16 threads, 16 elements each; the tile lives in shared memory
-// (row stride LX + LX/8) between the row phase (x transform, T = LX/16 consecutive threads per row, exchanges
+// (row stride LX + LX/16) between the row phase (x transform, T = LX/16 consecutive threads per row, exchanges
 // inside the row's warp) and the column phase (length-NY1 transform, lanes of a warp on adjacent columns).
 template <int RS> struct SmTileCol {
     static constexpr bool TWPOW = true;
@@ -436,7 +444,7 @@ __global__ void __launch_bounds__(LX *NY1 / 16, (LX * NY1 / 16 <= 256 ? 2 : 1))
     k_fft_xy(const c2 *__restrict__ in, c2 *__restrict__ out, const c2 *__restrict__ twx, const c2 *__restrict__ twy1, const c2 *__restrict__ twy,
              int ny, int rev, int ahead)
 {
-    constexpr int E = 16, TX = LX / E, RS = LX + LX / 8, T2 = NY1 / E;
+    constexpr int E = 16, TX = LX / E, RS = LX + LX / 16, T2 = NY1 / E;
     static_assert(LX >= 64 && NY1 >= 16, "tile too small for 16 elements per thread");
     extern __shared__ double2 smem[];
     const int ny0 = ny / NY1;
@@ -447,8 +455,8 @@ __global__ void __launch_bounds__(LX *NY1 / 16, (LX * NY1 / 16 <= 256 ? 2 : 1))
     const int t = threadIdx.x;
     const int r = t / TX, tid = t - r * TX;      // row phase
     const int tid2 = t / LX, kx = t - tid2 * LX; // column phase
-    SmLine<TX> sl{smem + r * RS, 1 + r};
-    SmTileCol<RS> sc{smem + kx + (kx >> 3)};
+    SmLine<TX, 4> sl{smem + r * RS, 1 + r};
+    SmTileCol<RS> sc{smem + kx + (kx >> 4)};
     c2 x[E];
     // One block per tile (a persistent block walking several tiles measured slower here: 58 against 52 us per pass on
     // 512x256x128).  While it computes, the block asks L2 for the tile of the block `ahead` places behind it in launch
@@ -465,7 +473,7 @@ __global__ void __launch_bounds__(LX *NY1 / 16, (LX * NY1 / 16 <= 256 ? 2 : 1))
 #pragma unroll
         for (int e = 0; e < E; ++e) x[e] = row[tid + e * TX];
         prefetch_next();
-        fft_line<LX, E, -1, 1, SmLine<TX>>(x, tid, twx, sl);
+        fft_line<LX, E, -1, 1, SmLine<TX, 4>>(x, tid, twx, sl);
 #pragma unroll
         for (int e = 0; e < E; ++e) sl.at(tid + e * TX) = x[e];
         __syncthreads();
@@ -494,7 +502,7 @@ __global__ void __launch_bounds__(LX *NY1 / 16, (LX * NY1 / 16 <= 256 ? 2 : 1))
 #pragma unroll
         for (int e = 0; e < E; ++e) x[e] = sl.at(tid + e * TX);
         sl.sync();
-        fft_line<LX, E, +1, 1, SmLine<TX>>(x, tid, twx, sl);
+        fft_line<LX, E, +1, 1, SmLine<TX, 4>>(x, tid, twx, sl);
         c2 *row = out + tile0 + r * rstride;
 #pragma unroll
         for (int e = 0; e < E; ++e) row[tid + e * TX] = x[e];
@@ -518,7 +526,7 @@ template <int N, int DIR> __device__ __forceinline__ void dft_small(c2 *v)
 }
 
 template <int STRIDE> struct SmStride {
-    static constexpr bool TWPOW = true;
+    static constexpr bool TWPOW = false, TWSMEM = true; // all lanes of a warp share a z butterfly: table look-ups broadcast
     c2 *base;
     __device__ __forceinline__ c2 &at(int n) { return base[n * STRIDE]; }
     __device__ __forceinline__ void sync() { __syncthreads(); }
@@ -527,35 +535,39 @@ template <int STRIDE> struct SmStride {
 template <int NY0, int LZ, int XT>
 __global__ void __launch_bounds__(XT *NY0 *LZ / 16, (XT * NY0 * LZ / 16 <= 256 ? 2 : 1))
     k_fft_yz_solve(c2 *__restrict__ data, const c2 *__restrict__ twz, int mx, int ny, const double *__restrict__ ex, const double *__restrict__ ey,
-                   const double *__restrict__ ez, double inv_n, int ntiles, int rev)
+                   const double *__restrict__ ez, double inv_n, int rev, int ahead)
 {
     constexpr int E = 16, G = E / NY0, ZQ = LZ / G, T = LZ / E, NT = XT * NY0 * LZ / E;
     // one z plane of the tile: NY0 XT numbers, padded so that the quarter-warps of both layouts hit 32 different banks
     constexpr int ZROW = NY0 * XT + (XT < 8 ? XT : 0);
     static_assert(NY0 >= 2 && NY0 <= 16 && LZ >= 32, "unsupported split");
     extern __shared__ double2 smem[];
-    double *sez = reinterpret_cast<double *>(smem + LZ * ZROW); // the z eigenvalue parts, read LZ times per tile
+    c2 *stw = smem + LZ * ZROW;                         // z twiddles exp(-2 pi i t/LZ)
+    double *sez = reinterpret_cast<double *>(stw + LZ); // z eigenvalue parts
     const int ny1 = ny / NY0, xtiles = mx / XT;
+    const unsigned bid = rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const int xt = bid % xtiles, ky1 = bid / xtiles;
     const int t = threadIdx.x, xl = t % XT, rest = t / XT;
     const int zq = rest;                          // first layout: all y0 of the planes zq + g ZQ
     const int ky0 = rest % NY0, tid = rest / NY0; // second layout: planes tid + e T of one ky0
     const size_t zstride = (size_t)mx * ny;
-    for (int q = t; q < LZ; q += NT) sez[q] = ez[q];
-    for (int lt = blockIdx.x; lt < ntiles; lt += gridDim.x) {
-        const unsigned bid = rev ? ntiles - 1 - lt : lt;
-        const int xt = bid % xtiles, ky1 = bid / xtiles;
-        c2 *g1 = data + (size_t)ky1 * NY0 * mx + (size_t)xt * XT + xl;
-        c2 x[E];
+    c2 *g1 = data + (size_t)ky1 * NY0 * mx + (size_t)xt * XT + xl;
+    c2 x[E];
 #pragma unroll
-        for (int g = 0; g < G; ++g)
+    for (int g = 0; g < G; ++g)
 #pragma unroll
-            for (int y0 = 0; y0 < NY0; ++y0) x[g * NY0 + y0] = g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx];
-        const int m = xt * XT + xl, ky = ky1 + ny1 * ky0;
-        const double exy = __ldg(&ex[m]) + __ldg(&ey[ky]);
-        if (lt + (int)gridDim.x < ntiles) {
-            // this block's next tile into L2 while this one is computed: LZ NY0 runs of XT complex numbers,
-            // one request per 128 bytes of each run
-            const unsigned nbid = rev ? ntiles - 1 - (lt + gridDim.x) : lt + gridDim.x;
+        for (int y0 = 0; y0 < NY0; ++y0) x[g * NY0 + y0] = g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx];
+    for (int q = t; q < LZ; q += NT) {
+        sez[q] = ez[q];
+        stw[q] = twz[q];
+    }
+    {
+        // While this tile is computed, ask L2 for the tile of the block `ahead` places behind in launch order (the one
+        // that takes over an SM about when this block retires): LZ NY0 runs of XT complex numbers, one request per
+        // 128 bytes of each run.
+        const unsigned nb = blockIdx.x + ahead;
+        if (ahead > 0 && nb < gridDim.x) {
+            const unsigned nbid = rev ? gridDim.x - 1 - nb : nb;
             const c2 *nt = data + (size_t)(nbid / xtiles) * NY0 * mx + (size_t)(nbid % xtiles) * XT;
             constexpr int PER_RUN = XT >= 8 ? XT / 8 : 1, RUNS = LZ * NY0, REQ = RUNS * PER_RUN;
 #pragma unroll
@@ -564,47 +576,47 @@ __global__ void __launch_bounds__(XT *NY0 *LZ / 16, (XT * NY0 * LZ / 16 <= 256 ?
                 if (q < REQ) prefetch_l2_line(nt + (size_t)(run / NY0) * zstride + (size_t)(run % NY0) * mx + part * 8);
             }
         }
-#pragma unroll
-        for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
-#pragma unroll
-        for (int g = 0; g < G; ++g)
-#pragma unroll
-            for (int q = 0; q < NY0; ++q) smem[(zq + g * ZQ) * ZROW + q * XT + xl] = x[g * NY0 + q];
-        __syncthreads();
-        SmStride<ZROW> sm{smem + ky0 * XT + xl};
-#pragma unroll
-        for (int e = 0; e < E; ++e) x[e] = sm.at(tid + e * T);
-        __syncthreads();
-        fft_line<LZ, E, -1, 1, SmStride<ZROW>>(x, tid, twz, sm);
-        {
-            const bool null_xy = (m == 0) && (((2 * ky) & (ny - 1)) == 0);
-#pragma unroll
-            for (int e = 0; e < E; ++e) {
-                const int kz = tid + e * T;
-                const double lam = -(exy + sez[kz]);
-                const bool null = null_xy && (((2 * kz) & (LZ - 1)) == 0);
-                const double sc = inv_n * rcp_newton(lam);
-                x[e].x = null ? 0.0 : x[e].x * sc;
-                x[e].y = null ? 0.0 : x[e].y * sc;
-            }
-        }
-        fft_line<LZ, E, +1, 1, SmStride<ZROW>>(x, tid, twz, sm);
-#pragma unroll
-        for (int e = 0; e < E; ++e) sm.at(tid + e * T) = x[e];
-        __syncthreads();
-#pragma unroll
-        for (int g = 0; g < G; ++g)
-#pragma unroll
-            for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = smem[(zq + g * ZQ) * ZROW + q * XT + xl];
-#pragma unroll
-        for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
-#pragma unroll
-        for (int g = 0; g < G; ++g)
-#pragma unroll
-            for (int y0 = 0; y0 < NY0; ++y0) g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx] = x[g * NY0 + y0];
-        // the first layout's slots are private to a thread (it reads back exactly what it wrote), so the next
-        // tile may start without another barrier
     }
+#pragma unroll
+    for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int q = 0; q < NY0; ++q) smem[(zq + g * ZQ) * ZROW + q * XT + xl] = x[g * NY0 + q];
+    __syncthreads();
+    SmStride<ZROW> sm{smem + ky0 * XT + xl};
+#pragma unroll
+    for (int e = 0; e < E; ++e) x[e] = sm.at(tid + e * T);
+    __syncthreads();
+    fft_line<LZ, E, -1, 1, SmStride<ZROW>>(x, tid, stw, sm);
+    {
+        const int m = xt * XT + xl, ky = ky1 + ny1 * ky0;
+        const double exy = __ldg(&ex[m]) + __ldg(&ey[ky]);
+        const bool null_xy = (m == 0) && (((2 * ky) & (ny - 1)) == 0);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int kz = tid + e * T;
+            const double lam = -(exy + sez[kz]);
+            const bool null = null_xy && (((2 * kz) & (LZ - 1)) == 0);
+            const double sc = inv_n * rcp_newton(lam);
+            x[e].x = null ? 0.0 : x[e].x * sc;
+            x[e].y = null ? 0.0 : x[e].y * sc;
+        }
+    }
+    fft_line<LZ, E, +1, 1, SmStride<ZROW>>(x, tid, stw, sm);
+#pragma unroll
+    for (int e = 0; e < E; ++e) sm.at(tid + e * T) = x[e];
+    __syncthreads();
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = smem[(zq + g * ZQ) * ZROW + q * XT + xl];
+#pragma unroll
+    for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int y0 = 0; y0 < NY0; ++y0) g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx] = x[g * NY0 + y0];
 }
 
 } // namespace dnsfft
