@@ -204,6 +204,8 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 __device__ __forceinline__ void cp_async_wait_one() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait_n() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
+template <bool B> struct BoolTag { static constexpr bool value = B; };
+
 // RHS of one cell for field m given its seven-point neighbourhood and the advecting velocities.
 template <bool MASKED_C>
 __device__ __forceinline__ double rk_rhs_cell(const RKArgs &a, int m, unsigned f, double c0, double xp, double xm, double yp, double ym,
@@ -238,48 +240,49 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
     const int by = a.rev ? gridDim.y - 1 - blockIdx.y : blockIdx.y, bz = a.rev ? gridDim.z - 1 - blockIdx.z : blockIdx.z;
     const int x0 = blockIdx.x * TX, y0 = by * RKM_TY, k0 = bz * kc;
     const int i = x0 + 2 * tx, j = y0 + ty;
-    const size_t plane = (size_t)nx * ny;
-    const size_t orow = (size_t)nx * j + i;
+    // element offsets are 32-bit (a field has at most 2^31 cells): one IMAD.WIDE per access instead of 64-bit chains
+    const unsigned plane = (unsigned)nx * (unsigned)ny;
+    const unsigned orow = (unsigned)nx * j + i;
 
     // this thread's share of one plane tile: per field 10 rows x 32 double2 (interior + y halo) and 20 x-halo values
     const int r_a = tid >> 5, q_a = tid & 31;                 // copy A: rows 0..7
-    const size_t src_a = (size_t)nx * ((y0 - 1 + r_a) & (ny - 1)) + x0 + 2 * q_a;
+    const unsigned src_a = (unsigned)nx * ((y0 - 1 + r_a) & (ny - 1)) + x0 + 2 * q_a;
     const int dst_a = r_a * SW + 2 + 2 * q_a;
     const bool has_b = tid < 64;                              // copy B: rows 8..9
-    const size_t src_b = (size_t)nx * ((y0 + 7 + r_a) & (ny - 1)) + x0 + 2 * q_a;
+    const unsigned src_b = (unsigned)nx * ((y0 + 7 + r_a) & (ny - 1)) + x0 + 2 * q_a;
     const int dst_b = (8 + r_a) * SW + 2 + 2 * q_a;
     const bool has_h = tid >= 64 && tid < 64 + 4 * ROWS * 2;  // x halo: 80 values
     const int hh = tid - 64, h_m = hh / (ROWS * 2), h_r = (hh % (ROWS * 2)) >> 1, h_s = hh & 1;
-    const size_t src_h = (size_t)nx * ((y0 - 1 + h_r) & (ny - 1)) + (h_s ? ((x0 + TX) & (nx - 1)) : ((x0 - 1) & (nx - 1)));
+    const unsigned src_h = (unsigned)nx * ((y0 - 1 + h_r) & (ny - 1)) + (h_s ? ((x0 + TX) & (nx - 1)) : ((x0 - 1) & (nx - 1)));
     const int dst_h = (h_m * ROWS + h_r) * SW + (h_s ? 2 + TX : 1);
+    const double *qs_h = has_h ? a.qs[h_m & 3] : a.qs[0];
     auto issue_plane = [&](int kk, int buf) {
-        const size_t pk = plane * (size_t)(kk & (nz - 1));
+        const unsigned pk = plane * (unsigned)(kk & (nz - 1));
         double *sb = sm + buf * PLANE;
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            cp_async16(sb + m * ROWS * SW + dst_a, a.qs[m] + pk + src_a);
-            if (has_b) cp_async16(sb + m * ROWS * SW + dst_b, a.qs[m] + pk + src_b);
+            cp_async16(sb + m * ROWS * SW + dst_a, a.qs[m] + (pk + src_a));
+            if (has_b) cp_async16(sb + m * ROWS * SW + dst_b, a.qs[m] + (pk + src_b));
         }
-        if (has_h) cp_async8(sb + dst_h, a.qs[h_m] + pk + src_h);
+        if (has_h) cp_async8(sb + dst_h, qs_h + (pk + src_h));
         cp_async_commit();
     };
 
 #pragma unroll
     for (int n = 0; n <= RKM_NBUF - 2; ++n) issue_plane(k0 + n, n);
-    // z-carried values of this thread's column: three register sets that take the roles z-1, centre, z+1 in
-    // turn (the plane loop is unrolled three times, so the carry is a renaming, not a copy)
-    double2 r0[4], r1[4], r2[4];
+    // z-carried values of this thread's column: z-1, centre, z+1 (rotated by copy at the end of every plane)
+    double2 zm[4], cur[4], zp[4];
     {
-        const size_t pkm = plane * (size_t)((k0 - 1) & (nz - 1));
+        const unsigned pkm = plane * (unsigned)((k0 - 1) & (nz - 1)) + orow;
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            r0[m] = __ldg(reinterpret_cast<const double2 *>(a.qs[m] + pkm + orow));
-            r1[m] = r2[m] = make_double2(0.0, 0.0);
+            zm[m] = __ldg(reinterpret_cast<const double2 *>(a.qs[m] + pkm));
+            cur[m] = zp[m] = make_double2(0.0, 0.0);
         }
     }
     const int own = (ty + 1) * SW + 2 + 2 * tx; // this thread's pair inside a field's tile
     unsigned fraw_next = 0x7f7f;
-    if (MASKED) fraw_next = *reinterpret_cast<const unsigned short *>(a.face + plane * (size_t)k0 + orow);
+    if (MASKED) fraw_next = *reinterpret_cast<const unsigned short *>(a.face + (plane * (unsigned)k0 + orow));
     // sources whose x and y factors are non-zero at this thread's cells (their z factor is checked per plane)
     unsigned smask = 0;
     if (SOURCES) {
@@ -289,16 +292,16 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
             if ((sx.x != 0.0 || sx.y != 0.0) && __ldg(&tb[nx + j]) != 0.0) smask |= 1u << s;
         }
     }
+    const RhsCoef &kf = a.kf;
 
-    auto plane_step = [&](const int t, double2 (&zm)[4], double2 (&cur)[4], double2 (&zp)[4]) {
+    for (int t = 0; t < kc; ++t) {
         const int k = k0 + t;
-        const size_t o = plane * (size_t)k + orow;
+        const unsigned o = plane * (unsigned)k + orow;
         // operands that do not go through shared memory: issue their loads before waiting
         double2 qn[4], q2[4];
         // face bytes: fetched one plane ahead and left packed until here, so the load is never waited for
         const unsigned fraw = fraw_next;
-        if (MASKED && t + 1 < kc) fraw_next = *reinterpret_cast<const unsigned short *>(a.face + o + plane);
-        const unsigned fA = fraw & 0xffu, fB = fraw >> 8;
+        if (MASKED && t + 1 < kc) fraw_next = *reinterpret_cast<const unsigned short *>(a.face + (o + plane));
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
             if (STAGE >= 2 && (STAGE <= 3 || !ELIM)) qn[m] = __ldg(reinterpret_cast<const double2 *>(a.qn[m] + o));
@@ -322,7 +325,6 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
         }
         // factored form of the right-hand side: per cell six coefficients shared by the four fields
         //   A+-_a = -(u_a(+-a) + u_a)/(4 Delta_a), then F = sum_a [q(+a)(A+_a + D_a) + q(-a)(D_a - A-_a)] - 2 sum_a D_a q0 + b
-        const RhsCoef &kf = a.kf;
         double axp[2], axm[2], ayp[2], aym[2], azp[2], azm[2];
         {
             const double2 vym = *reinterpret_cast<const double2 *>(sC + 1 * ROWS * SW + own - SW);
@@ -335,122 +337,131 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
             azp[0] = (zp[2].x + cur[2].x) * kf.hz; azm[0] = (zm[2].x + cur[2].x) * kf.hz;
             azp[1] = (zp[2].y + cur[2].y) * kf.hz; azm[1] = (zm[2].y + cur[2].y) * kf.hz;
         }
-        double2 F[4];
-        {
-            // scalar first: its diffusive coefficients carry the face bits of eq. 4
-            const double *sf = sC + 3 * ROWS * SW + own;
-            const double2 ym = *reinterpret_cast<const double2 *>(sf - SW), yp = *reinterpret_cast<const double2 *>(sf + SW);
-            const double xpv[2] = {cur[3].y, sf[2]}, xmv[2] = {sf[-1], cur[3].x};
-            const double ypv[2] = {yp.x, yp.y}, ymv[2] = {ym.x, ym.y}, zpv[2] = {zp[3].x, zp[3].y}, zmv[2] = {zm[3].x, zm[3].y};
-            const double c0v[2] = {cur[3].x, cur[3].y};
-            const unsigned fv[2] = {fA, fB};
-            double out[2];
+        // The rest of the plane in two versions chosen per warp (no divergence): WALL = some cell of this warp's row
+        // has a solid cell in its seven-point neighbourhood.  Nine warps in ten of a room see none and run without a
+        // single select (the face-weighted diffusion of eq. 4 and the beta ? x : +0.0 of PAPER.md:58 cost 20 selects per
+        // cell); both versions give the same bits for an all-fluid neighbourhood.
+        auto finish = [&](auto wall_tag) {
+            constexpr bool WALL = decltype(wall_tag)::value;
+            const unsigned fA = fraw & 0xffu, fB = fraw >> 8;
+            double2 F[4];
+            {
+                // scalar first: its diffusive coefficients carry the face bits of eq. 4
+                const double *sf = sC + 3 * ROWS * SW + own;
+                const double2 ym = *reinterpret_cast<const double2 *>(sf - SW), yp = *reinterpret_cast<const double2 *>(sf + SW);
+                const double xpv[2] = {cur[3].y, sf[2]}, xmv[2] = {sf[-1], cur[3].x};
+                const double ypv[2] = {yp.x, yp.y}, ymv[2] = {ym.x, ym.y}, zpv[2] = {zp[3].x, zp[3].y}, zmv[2] = {zm[3].x, zm[3].y};
+                const double c0v[2] = {cur[3].x, cur[3].y};
+                const unsigned fv[2] = {fA, fB};
+                double out[2];
+#pragma unroll
+                for (int l = 0; l < 2; ++l) {
+                    double v;
+                    if (!WALL) {
+                        v = kf.dc0 * c0v[l];
+                        v = fma(xpv[l], axp[l] + kf.dcx, v);
+                        v = fma(xmv[l], kf.dcx - axm[l], v);
+                        v = fma(ypv[l], ayp[l] + kf.dcy, v);
+                        v = fma(ymv[l], kf.dcy - aym[l], v);
+                        v = fma(zpv[l], azp[l] + kf.dcz, v);
+                        v = fma(zmv[l], kf.dcz - azm[l], v);
+                    } else {
+                        const unsigned fl = fv[l];
+                        const double exp_ = (fl & 2) ? kf.dcx : 0.0, exm = (fl & 4) ? kf.dcx : 0.0;
+                        const double eyp = (fl & 8) ? kf.dcy : 0.0, eym = (fl & 16) ? kf.dcy : 0.0;
+                        const double ezp = (fl & 32) ? kf.dcz : 0.0, ezm = (fl & 64) ? kf.dcz : 0.0;
+                        v = -(((exp_ + exm) + (eyp + eym)) + (ezp + ezm)) * c0v[l];
+                        v = fma(xpv[l], axp[l] + exp_, v);
+                        v = fma(xmv[l], exm - axm[l], v);
+                        v = fma(ypv[l], ayp[l] + eyp, v);
+                        v = fma(ymv[l], eym - aym[l], v);
+                        v = fma(zpv[l], azp[l] + ezp, v);
+                        v = fma(zmv[l], ezm - azm[l], v);
+                    }
+                    out[l] = v;
+                }
+                F[3] = make_double2(out[0], out[1]);
+            }
+            double bxp[2], bxm[2], byp[2], bym[2], bzp[2], bzm[2];
 #pragma unroll
             for (int l = 0; l < 2; ++l) {
-                double v;
-                if (!MASKED) {
-                    v = kf.dc0 * c0v[l];
-                    v = fma(xpv[l], axp[l] + kf.dcx, v);
-                    v = fma(xmv[l], kf.dcx - axm[l], v);
-                    v = fma(ypv[l], ayp[l] + kf.dcy, v);
-                    v = fma(ymv[l], kf.dcy - aym[l], v);
-                    v = fma(zpv[l], azp[l] + kf.dcz, v);
-                    v = fma(zmv[l], kf.dcz - azm[l], v);
-                } else {
-                    const unsigned fl = fv[l];
-                    const double exp_ = (fl & 2) ? kf.dcx : 0.0, exm = (fl & 4) ? kf.dcx : 0.0;
-                    const double eyp = (fl & 8) ? kf.dcy : 0.0, eym = (fl & 16) ? kf.dcy : 0.0;
-                    const double ezp = (fl & 32) ? kf.dcz : 0.0, ezm = (fl & 64) ? kf.dcz : 0.0;
-                    v = -(((exp_ + exm) + (eyp + eym)) + (ezp + ezm)) * c0v[l];
-                    v = fma(xpv[l], axp[l] + exp_, v);
-                    v = fma(xmv[l], exm - axm[l], v);
-                    v = fma(ypv[l], ayp[l] + eyp, v);
-                    v = fma(ymv[l], eym - aym[l], v);
-                    v = fma(zpv[l], azp[l] + ezp, v);
-                    v = fma(zmv[l], ezm - azm[l], v);
+                bxp[l] = axp[l] + kf.dvx; bxm[l] = kf.dvx - axm[l];
+                byp[l] = ayp[l] + kf.dvy; bym[l] = kf.dvy - aym[l];
+                bzp[l] = azp[l] + kf.dvz; bzm[l] = kf.dvz - azm[l];
+            }
+#pragma unroll
+            for (int m = 0; m < 3; ++m) {
+                const double *sf = sC + m * ROWS * SW + own;
+                const double2 ym = *reinterpret_cast<const double2 *>(sf - SW), yp = *reinterpret_cast<const double2 *>(sf + SW);
+                const double xmA = sf[-1], xpB = sf[2];
+                double vx = fma(kf.dv0, cur[m].x, a.body[m]), vy = fma(kf.dv0, cur[m].y, a.body[m]);
+                vx = fma(cur[m].y, bxp[0], vx); vy = fma(xpB, bxp[1], vy);
+                vx = fma(xmA, bxm[0], vx);      vy = fma(cur[m].x, bxm[1], vy);
+                vx = fma(yp.x, byp[0], vx);     vy = fma(yp.y, byp[1], vy);
+                vx = fma(ym.x, bym[0], vx);     vy = fma(ym.y, bym[1], vy);
+                vx = fma(zp[m].x, bzp[0], vx);  vy = fma(zp[m].y, bzp[1], vy);
+                vx = fma(zm[m].x, bzm[0], vx);  vy = fma(zm[m].y, bzm[1], vy);
+                F[m] = make_double2(vx, vy);
+            }
+            if (SOURCES) {
+                for (unsigned sm_ = smask; sm_; sm_ &= sm_ - 1) {
+                    const int s = __ffs(sm_) - 1;
+                    const double *tb = a.stab + a.src[s].off;
+                    const double sz = __ldg(&tb[nx + ny + k]), sy = __ldg(&tb[nx + j]);
+                    if (sz == 0.0) continue;
+                    const double2 sx = __ldg(reinterpret_cast<const double2 *>(tb + i));
+                    const double SA = sx.x * sy * sz, SB = sx.y * sy * sz;
+                    const uint32_t comps = a.src[s].comps;
+#pragma unroll
+                    for (int m = 0; m < 4; ++m)
+                        if (comps & (1u << m)) {
+                            if (SA != 0.0) F[m].x += SA * (a.src[s].set[m] - cur[m].x) * a.src[s].rtau;
+                            if (SB != 0.0) F[m].y += SB * (a.src[s].set[m] - cur[m].y) * a.src[s].rtau;
+                        }
                 }
-                out[l] = v;
             }
-            F[3] = make_double2(out[0], out[1]);
-        }
+            const bool flA = !WALL || (fA & 1), flB = !WALL || (fB & 1);
 #pragma unroll
-        for (int l = 0; l < 2; ++l) {
-            axp[l] = axp[l] + kf.dvx; axm[l] = kf.dvx - axm[l];
-            ayp[l] = ayp[l] + kf.dvy; aym[l] = kf.dvy - aym[l];
-            azp[l] = azp[l] + kf.dvz; azm[l] = kf.dvz - azm[l];
-        }
-#pragma unroll
-        for (int m = 0; m < 3; ++m) {
-            const double *sf = sC + m * ROWS * SW + own;
-            const double2 ym = *reinterpret_cast<const double2 *>(sf - SW), yp = *reinterpret_cast<const double2 *>(sf + SW);
-            const double xmA = sf[-1], xpB = sf[2];
-            double vx = fma(kf.dv0, cur[m].x, a.body[m]), vy = fma(kf.dv0, cur[m].y, a.body[m]);
-            vx = fma(cur[m].y, axp[0], vx); vy = fma(xpB, axp[1], vy);
-            vx = fma(xmA, axm[0], vx);      vy = fma(cur[m].x, axm[1], vy);
-            vx = fma(yp.x, ayp[0], vx);     vy = fma(yp.y, ayp[1], vy);
-            vx = fma(ym.x, aym[0], vx);     vy = fma(ym.y, aym[1], vy);
-            vx = fma(zp[m].x, azp[0], vx);  vy = fma(zp[m].y, azp[1], vy);
-            vx = fma(zm[m].x, azm[0], vx);  vy = fma(zm[m].y, azm[1], vy);
-            F[m] = make_double2(vx, vy);
-        }
-        if (SOURCES) {
-            for (unsigned sm_ = smask; sm_; sm_ &= sm_ - 1) {
-                const int s = __ffs(sm_) - 1;
-                const double *tb = a.stab + a.src[s].off;
-                const double sz = __ldg(&tb[nx + ny + k]), sy = __ldg(&tb[nx + j]);
-                if (sz == 0.0) continue;
-                const double2 sx = __ldg(reinterpret_cast<const double2 *>(tb + i));
-                const double SA = sx.x * sy * sz, SB = sx.y * sy * sz;
-                const uint32_t comps = a.src[s].comps;
-#pragma unroll
-                for (int m = 0; m < 4; ++m)
-                    if (comps & (1u << m)) {
-                        if (SA != 0.0) F[m].x += SA * (a.src[s].set[m] - cur[m].x) * a.src[s].rtau;
-                        if (SB != 0.0) F[m].y += SB * (a.src[s].set[m] - cur[m].y) * a.src[s].rtau;
+            for (int m = 0; m < 4; ++m) {
+                // solid cell: every field it holds is +0.0 and stays +0.0 (select)
+                if (ELIM) {
+                    double2 r;
+                    if (STAGE < 4) {
+                        r.x = flA ? qn[m].x + a.ca * F[m].x : 0.0;
+                        r.y = flB ? qn[m].y + a.ca * F[m].y : 0.0;
+                        *reinterpret_cast<double2 *>(a.qo[m] + o) = r;
+                        if (STAGE == 2) { // S = Q2 - Qn + 2 Q3 (all +0.0 in solid cells)
+                            double2 sv;
+                            sv.x = flA ? (cur[m].x - qn[m].x) + 2.0 * r.x : 0.0;
+                            sv.y = flB ? (cur[m].y - qn[m].y) + 2.0 * r.y : 0.0;
+                            *reinterpret_cast<double2 *>(a.qco[m] + o) = sv;
+                        }
+                    } else {
+                        r.x = flA ? (q2[m].x + cur[m].x) * (1.0 / 3.0) + a.cb * F[m].x : 0.0;
+                        r.y = flB ? (q2[m].y + cur[m].y) * (1.0 / 3.0) + a.cb * F[m].y : 0.0;
+                        *reinterpret_cast<double2 *>(a.qco[m] + o) = r;
                     }
+                } else {
+                    double2 c, r;
+                    const double2 qcv = STAGE >= 2 ? q2[m] : qn[m];
+                    c.x = flA ? qcv.x + a.cb * F[m].x : 0.0;
+                    c.y = flB ? qcv.y + a.cb * F[m].y : 0.0;
+                    *reinterpret_cast<double2 *>(a.qco[m] + o) = c;
+                    if (STAGE < 4) {
+                        r.x = flA ? qn[m].x + a.ca * F[m].x : 0.0;
+                        r.y = flB ? qn[m].y + a.ca * F[m].y : 0.0;
+                        *reinterpret_cast<double2 *>(a.qo[m] + o) = r;
+                    }
+                }
             }
-        }
-        const bool flA = !MASKED || (fA & 1), flB = !MASKED || (fB & 1);
+        };
+        if (MASKED && __any_sync(0xffffffffu, fraw != 0x7f7fu)) finish(BoolTag<true>{});
+        else finish(BoolTag<false>{});
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            // solid cell: every field it holds is +0.0 and stays +0.0 (select)
-            if (ELIM) {
-                double2 r;
-                if (STAGE < 4) {
-                    r.x = flA ? qn[m].x + a.ca * F[m].x : 0.0;
-                    r.y = flB ? qn[m].y + a.ca * F[m].y : 0.0;
-                    *reinterpret_cast<double2 *>(a.qo[m] + o) = r;
-                    if (STAGE == 2) { // S = Q2 - Qn + 2 Q3 (all +0.0 in solid cells)
-                        double2 sv;
-                        sv.x = flA ? (cur[m].x - qn[m].x) + 2.0 * r.x : 0.0;
-                        sv.y = flB ? (cur[m].y - qn[m].y) + 2.0 * r.y : 0.0;
-                        *reinterpret_cast<double2 *>(a.qco[m] + o) = sv;
-                    }
-                } else {
-                    r.x = flA ? (q2[m].x + cur[m].x) * (1.0 / 3.0) + a.cb * F[m].x : 0.0;
-                    r.y = flB ? (q2[m].y + cur[m].y) * (1.0 / 3.0) + a.cb * F[m].y : 0.0;
-                    *reinterpret_cast<double2 *>(a.qco[m] + o) = r;
-                }
-            } else {
-                double2 c, r;
-                const double2 qcv = STAGE >= 2 ? q2[m] : qn[m];
-                c.x = flA ? qcv.x + a.cb * F[m].x : 0.0;
-                c.y = flB ? qcv.y + a.cb * F[m].y : 0.0;
-                *reinterpret_cast<double2 *>(a.qco[m] + o) = c;
-                if (STAGE < 4) {
-                    r.x = flA ? qn[m].x + a.ca * F[m].x : 0.0;
-                    r.y = flB ? qn[m].y + a.ca * F[m].y : 0.0;
-                    *reinterpret_cast<double2 *>(a.qo[m] + o) = r;
-                }
-            }
+            zm[m] = cur[m];
+            cur[m] = zp[m];
         }
-    };
-    for (int t = 0; t < kc; t += 3) {
-        plane_step(t, r0, r1, r2);
-        if (t + 1 >= kc) break;
-        plane_step(t + 1, r1, r2, r0);
-        if (t + 2 >= kc) break;
-        plane_step(t + 2, r2, r0, r1);
     }
 }
 
