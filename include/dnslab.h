@@ -100,6 +100,17 @@ int dnslab_step(dnslab_t *h, int32_t n);
  * touch the solver's own pressure. */
 int dnslab_poisson(dnslab_t *h, const double *rhs, double *p);
 
+/* The transform of the solve on its own (testing aid: north_star names a real-to-complex transform; the solve itself
+ * never forms this spectrum -- it transforms the packed array and divides by the even eigenvalue table).
+ * dnslab_rfft3: in = nx*ny*nz doubles (DEVICE); out = (nx/2+1)*ny*nz complex numbers (re, im interleaved, DEVICE),
+ *   out[m + (nx/2+1)*(ky + ny*kz)] = sum_{i,j,k} in[i + nx*(j + ny*k)] exp(-2 pi i (m i/nx + ky j/ny + kz k/nz)),
+ *   unnormalised, m = 0..nx/2.  Computed with the single-axis passes of the solve (x, y, z) plus one untangling kernel.
+ * dnslab_irfft3: the inverse (in = such a half spectrum, Hermitian; out = nx*ny*nz doubles), includes the 1/N.
+ * in and out must not overlap.  Both use the solver's work array: do not call between dnslab_step launches on
+ * another stream.  PAPER.md:43 ("fft"), eq. 9 PAPER.md:102. */
+int dnslab_rfft3(dnslab_t *h, const double *in, double *out);
+int dnslab_irfft3(dnslab_t *h, const double *in, double *out);
+
 /* Borrowed DEVICE pointers to the current u,v,w,c,p (any out-pointer may be NULL).  No copy.
  * Valid until the next dnslab_step / dnslab_set_fields / dnslab_destroy (buffers rotate). */
 int dnslab_fields(dnslab_t *h, const double **u, const double **v, const double **w, const double **c,

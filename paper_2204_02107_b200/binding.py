@@ -11,7 +11,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdnslab.so")
 
 SYMBOLS = ["dnslab_workspace_bytes", "dnslab_create", "dnslab_set_fields", "dnslab_step", "dnslab_poisson",
-           "dnslab_fields", "dnslab_get_fields", "dnslab_launch_count", "dnslab_profile", "dnslab_profile_read",
+           "dnslab_rfft3", "dnslab_irfft3", "dnslab_fields", "dnslab_get_fields", "dnslab_launch_count", "dnslab_profile", "dnslab_profile_read",
            "dnslab_courant", "dnslab_set_dt", "dnslab_scalar_stats", "dnslab_particles_attach", "dnslab_destroy", "dnslab_strerror"]
 KERNEL_CLASSES = ["rk_stage", "div", "fft_x", "fft_y", "fft_z_solve", "project", "eq9_sparse", "filter", "reduce", "particles",
                   "fft_xy", "fft_yz_solve"]
@@ -52,6 +52,8 @@ def lib():
         L.dnslab_set_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 5
         L.dnslab_step.argtypes = [C.c_void_p, C.c_int32]
         L.dnslab_poisson.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.dnslab_rfft3.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.dnslab_irfft3.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.dnslab_fields.argtypes = [C.c_void_p] + [C.POINTER(C.c_void_p)] * 5
         L.dnslab_get_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 5
         L.dnslab_launch_count.argtypes = [C.c_void_p]
@@ -165,6 +167,23 @@ class Solver:
         if out is None:
             out = torch.empty_like(rhs)
         _check(lib().dnslab_poisson(self._h, rhs.data_ptr(), out.data_ptr()), "dnslab_poisson")
+        return out
+
+    def rfft3(self, x):
+        """dnslab_rfft3: x float64 CUDA (nz, ny, nx) -> complex128 CUDA (nz, ny, nx/2 + 1), unnormalised."""
+        torch = self._torch
+        assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous() and tuple(x.shape) == self.shape
+        out = torch.empty(self.shape[:2] + (self.shape[2] // 2 + 1,), dtype=torch.complex128, device=x.device)
+        _check(lib().dnslab_rfft3(self._h, x.data_ptr(), out.data_ptr()), "dnslab_rfft3")
+        return out
+
+    def irfft3(self, X):
+        """dnslab_irfft3: complex128 CUDA (nz, ny, nx/2 + 1) -> float64 CUDA (nz, ny, nx), includes 1/N."""
+        torch = self._torch
+        assert X.is_cuda and X.dtype == torch.complex128 and X.is_contiguous()
+        assert tuple(X.shape) == self.shape[:2] + (self.shape[2] // 2 + 1,)
+        out = torch.empty(self.shape, dtype=torch.float64, device=X.device)
+        _check(lib().dnslab_irfft3(self._h, X.data_ptr(), out.data_ptr()), "dnslab_irfft3")
         return out
 
     def field_ptrs(self):

@@ -647,6 +647,17 @@ int prepare_kernels(dnslab *h)
     }
     if ((rc = poisson_solve(h, h->d, h->p, h->p, true))) return rc;
     if ((rc = poisson_solve(h, h->d, h->p, h->p, false))) return rc; // dnslab_poisson: never the dense prologue
+    {
+        // dnslab_rfft3 / dnslab_irfft3 always take the single-axis passes, along z too
+        const int keep = h->f_ny1;
+        h->f_ny1 = 0;
+        rc = poisson_solve(h, h->d, h->p, h->p, false);
+        h->f_ny1 = keep;
+        if (rc) return rc;
+        c2 *W = reinterpret_cast<c2 *>(h->W);
+        if ((rc = launch_fft_col<-1>(h, W, 2))) return rc;
+        if ((rc = launch_fft_col<+1>(h, W, 2))) return rc;
+    }
     if ((h->P.flags & 1u) && (rc = launch_filter(h, h->Qc, h->A))) return rc;
     return DNSLAB_OK;
 }
@@ -931,6 +942,37 @@ int dnslab_poisson(dnslab_t *h, const double *rhs, double *p)
     return poisson_solve(h, rhs, nullptr, p, false);
 }
 
+int dnslab_rfft3(dnslab_t *h, const double *in, double *out)
+{
+    if (!h || !in || !out) return DNSLAB_EINVAL;
+    const int M = h->P.nx / 2;
+    dnsfft::PoissonRhsArgs ra{};
+    c2 *W = reinterpret_cast<c2 *>(h->W);
+    int rc;
+    if ((rc = launch_fft_x<-1, false>(h, reinterpret_cast<const c2 *>(in), W, ra))) return rc;
+    if ((rc = launch_fft_col<-1>(h, W, 1))) return rc;
+    if ((rc = launch_fft_col<-1>(h, W, 2))) return rc;
+    const size_t total = (size_t)(M + 1) * h->P.ny * h->P.nz;
+    dnsfft::k_r2c_tangle<<<(unsigned)((total + 255) / 256), 256, 0, h->stream>>>(W, reinterpret_cast<c2 *>(out), M, h->P.ny, h->P.nz, 0, 1.0);
+    return check_launch(h);
+}
+
+int dnslab_irfft3(dnslab_t *h, const double *in, double *out)
+{
+    if (!h || !in || !out) return DNSLAB_EINVAL;
+    const int M = h->P.nx / 2;
+    dnsfft::PoissonRhsArgs ra{};
+    c2 *W = reinterpret_cast<c2 *>(h->W);
+    const size_t total = (size_t)M * h->P.ny * h->P.nz;
+    dnsfft::k_r2c_tangle<<<(unsigned)((total + 255) / 256), 256, 0, h->stream>>>(reinterpret_cast<const c2 *>(in), W, M, h->P.ny, h->P.nz, 1,
+                                                                                  1.0 / (double)total);
+    int rc;
+    if ((rc = check_launch(h))) return rc;
+    if ((rc = launch_fft_col<+1>(h, W, 2))) return rc;
+    if ((rc = launch_fft_col<+1>(h, W, 1))) return rc;
+    return launch_fft_x<+1, false>(h, W, reinterpret_cast<c2 *>(out), ra);
+}
+
 int dnslab_fields(dnslab_t *h, const double **u, const double **v, const double **w, const double **c, const double **p)
 {
     if (!h) return DNSLAB_EINVAL;
@@ -1035,23 +1077,24 @@ int dnslab_scalar_stats(dnslab_t *h, const int32_t lo[3], const int32_t size[3],
         a.size[d] = size[d];
         a.count *= (size_t)size[d];
     }
-    // W (scratch outside a solve): res[0..3], then 2 G partials
+    // W (scratch outside a solve): res[0..3], then 2 G partials; a block takes whole rows of the box
     double *res = h->W, *part = h->W + 8;
-    size_t G = (a.count + 4095) / 4096;
-    const size_t gmax = (size_t)8 * h->nsm < (h->n - 8) / 2 ? (size_t)8 * h->nsm : (h->n - 8) / 2;
-    if (G > gmax) G = gmax;
-    if (G < 1) G = 1;
-    const size_t chunk = (a.count + G - 1) / G;
+    const unsigned rows = (unsigned)size[1] * (unsigned)size[2];
+    unsigned G = (unsigned)(16 * h->nsm);
+    if (G > rows) G = rows;
+    if (2 * (size_t)G + 8 > h->n) G = (unsigned)((h->n - 8) / 2);
+    const unsigned rpb = (rows + G - 1) / G;
+    G = (rows + rpb - 1) / rpb;
     {
         ProfScope ps(h, DNSLAB_K_REDUCE);
-        dnsred::k_box_partial<0><<<(unsigned)G, 256, 0, h->stream>>>(a, chunk, res, part);
+        dnsred::k_box_partial<0><<<G, 256, 0, h->stream>>>(a, rows, rpb, res, part);
         if (int rc = check_launch(h)) return rc;
     }
     dnsred::k_box_final<0><<<1, 256, 0, h->stream>>>(part, (int)G, res);
     if (int rc = check_launch(h)) return rc;
     {
         ProfScope ps(h, DNSLAB_K_REDUCE);
-        dnsred::k_box_partial<1><<<(unsigned)G, 256, 0, h->stream>>>(a, chunk, res, part);
+        dnsred::k_box_partial<1><<<G, 256, 0, h->stream>>>(a, rows, rpb, res, part);
         if (int rc = check_launch(h)) return rc;
     }
     dnsred::k_box_final<1><<<1, 256, 0, h->stream>>>(part, (int)G, res);

@@ -439,8 +439,11 @@ template <int RS> struct SmTileCol {
     __device__ __forceinline__ void sync() { __syncthreads(); }
 };
 
+#ifndef DNSLAB_XY_MINB
+#define DNSLAB_XY_MINB 2
+#endif
 template <int LX, int NY1, int DIR>
-__global__ void __launch_bounds__(LX *NY1 / 16, (LX * NY1 / 16 <= 256 ? 2 : 1))
+__global__ void __launch_bounds__(LX *NY1 / 16, (LX * NY1 / 16 <= 256 ? DNSLAB_XY_MINB : 1))
     k_fft_xy(const c2 *__restrict__ in, c2 *__restrict__ out, const c2 *__restrict__ twx, const c2 *__restrict__ twy1, const c2 *__restrict__ twy,
              int ny, int rev, int ahead)
 {
@@ -617,6 +620,42 @@ __global__ void __launch_bounds__(XT *NY0 *LZ / 16, (XT * NY0 * LZ / 16 <= 256 ?
     for (int g = 0; g < G; ++g)
 #pragma unroll
         for (int y0 = 0; y0 < NY0; ++y0) g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx] = x[g * NY0 + y0];
+}
+
+// ---------------------------------------------------------------------------------------
+// Real-to-complex entry points (dnslab_rfft3 / dnslab_irfft3): the transform itself, apart from the solve.
+// The packed array z[i'] = x[2i'] + i x[2i'+1] (M = nx/2 complex numbers per row) has the transform Z = E + iO,
+// E and O the transforms of the even and odd real sub-sequences; with Hermitian symmetry of both,
+//   E[m] = (Z[m] + conj Z[-m])/2,  O[m] = (Z[m] - conj Z[-m])/(2i)   (-m: all three indices negated, modulo M, ny, nz)
+// and the real-to-complex result is X[m] = E[m] + exp(-2 pi i m/nx) O[m] for m = 0..M (M+1 numbers per row).
+// inverse = false: Z (M per row) -> X (M+1 per row).  inverse = true: X -> scale * Z, ready for the inverse passes.
+__global__ void __launch_bounds__(256) k_r2c_tangle(const c2 *__restrict__ in, c2 *__restrict__ out, int M, int ny, int nz, int inverse,
+                                                    double scale)
+{
+    const int mcount = inverse ? M : M + 1;
+    const size_t total = (size_t)mcount * ny * nz, q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= total) return;
+    const int m = (int)(q % mcount), ky = (int)((q / mcount) % ny), kz = (int)(q / ((size_t)mcount * ny));
+    const int nky = (ny - ky) & (ny - 1), nkz = (nz - kz) & (nz - 1);
+    double sn, cs;
+    sincospi(-(double)m / (double)M, &sn, &cs); // w = exp(-i pi m/M) = exp(-2 pi i m/nx)
+    if (!inverse) {
+        const c2 a = in[(size_t)(m & (M - 1)) + (size_t)M * (ky + (size_t)ny * kz)];
+        c2 b = in[(size_t)((M - m) & (M - 1)) + (size_t)M * (nky + (size_t)ny * nkz)];
+        b.y = -b.y;
+        const c2 E = make_double2(0.5 * (a.x + b.x), 0.5 * (a.y + b.y));
+        const c2 O = make_double2(0.5 * (a.y - b.y), -0.5 * (a.x - b.x)); // (a - b)/(2i)
+        out[q] = make_double2(E.x + (cs * O.x - sn * O.y), E.y + (cs * O.y + sn * O.x));
+    } else {
+        const int R = M + 1;
+        const c2 a = in[(size_t)m + (size_t)R * (ky + (size_t)ny * kz)];
+        c2 b = in[(size_t)(M - m) + (size_t)R * (nky + (size_t)ny * nkz)];
+        b.y = -b.y;
+        const c2 E = make_double2(0.5 * (a.x + b.x), 0.5 * (a.y + b.y));
+        const c2 D = make_double2(0.5 * (a.x - b.x), 0.5 * (a.y - b.y));
+        const c2 O = make_double2(D.x * cs + D.y * sn, D.y * cs - D.x * sn); // D conj(w), conj(w) = cs - i sn
+        out[q] = make_double2(scale * (E.x - O.y), scale * (E.y + O.x));     // scale (E + i O)
+    }
 }
 
 } // namespace dnsfft

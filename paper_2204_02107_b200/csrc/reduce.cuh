@@ -8,18 +8,49 @@
 
 namespace dnsred {
 
-// max over all cells of |u|/dx + |v|/dy + |w|/dz (reading R24).  Divisions and the order of the
-// sum are those of the definition, so the value is bit-identical to a plain loop; the bit pattern of a
-// non-negative double orders like an unsigned integer, which makes the maximum an integer atomicMax.
-// A NaN rate never compares greater and is skipped, as in `if (r > best) best = r`.
+// max over all cells of |u|/dx + |v|/dy + |w|/dz (reading R24), bit-identical to a plain loop of that
+// expression.  Three correctly rounded fp64 divisions per cell would make this a compute-bound kernel (132 us on
+// 512x256x128 against 62 us for its one read of u, v, w), so every cell is first rated with reciprocal multiplies
+// (|u| rx + |v| ry + |w| rz, within 1e-15 relative of the exact expression: all terms are non-negative), and the
+// exact expression with its divisions is evaluated only where that rating comes within 1e-14 of the largest rating
+// the WARP has seen so far -- which always includes the cell of the true maximum, and happens O(log n) times per warp
+// (a per-thread threshold would make some lane of the warp take the slow path at almost every step).
+// The bit pattern of a non-negative double orders like an unsigned integer, which makes the final maximum an integer
+// atomicMax.  A NaN rate never compares greater and is skipped, as in `if (r > best) best = r`.
 __global__ void __launch_bounds__(256) k_courant(const double *__restrict__ u, const double *__restrict__ v, const double *__restrict__ w,
                                                  size_t n, double dx, double dy, double dz, unsigned long long *__restrict__ out)
 {
-    double best = 0.0;
-    for (size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (size_t)gridDim.x * blockDim.x) {
-        const double r = fabs(u[o]) / dx + fabs(v[o]) / dy + fabs(w[o]) / dz;
+    const double rx = 1.0 / dx, ry = 1.0 / dy, rz = 1.0 / dz;
+    double best = 0.0, rated = 0.0; // exact maximum of this thread's cells so far; largest rating of the warp so far
+    auto rate = [&](double uu, double vv, double ww) { return fma(fabs(ww), rz, fma(fabs(vv), ry, fabs(uu) * rx)); };
+    auto exact = [&](double uu, double vv, double ww) {
+        const double r = fabs(uu) / dx + fabs(vv) / dy + fabs(ww) / dz;
         if (r > best) best = r;
+    };
+    const size_t n2 = n / 2, stride = (size_t)gridDim.x * blockDim.x;
+    const double2 *u2 = reinterpret_cast<const double2 *>(u), *v2 = reinterpret_cast<const double2 *>(v), *w2 = reinterpret_cast<const double2 *>(w);
+    // whole warps enter or leave the loop together: the bound is rounded up to a multiple of 32 and lanes past the end idle
+    const size_t first = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (size_t o = first; o - (threadIdx.x & 31) < n2; o += stride) {
+        double2 a = make_double2(0.0, 0.0), b = a, c = a;
+        if (o < n2) {
+            a = __ldg(u2 + o);
+            b = __ldg(v2 + o);
+            c = __ldg(w2 + o);
+        }
+        const double q0 = rate(a.x, b.x, c.x), q1 = rate(a.y, b.y, c.y);
+        const double thr = rated * (1.0 - 1e-14);
+        const bool t0 = q0 >= thr, t1 = q1 >= thr;
+        if (__any_sync(0xffffffffu, t0 || t1)) {
+            if (t0) exact(a.x, b.x, c.x);
+            if (t1) exact(a.y, b.y, c.y);
+            double m = fmax(rated, fmax(q0, q1)); // fmax ignores a NaN rating
+#pragma unroll
+            for (int s = 16; s > 0; s >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, s));
+            rated = m;
+        }
     }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) exact(u[n - 1], v[n - 1], w[n - 1]);
     unsigned long long b = (unsigned long long)__double_as_longlong(best);
 #pragma unroll
     for (int s = 16; s > 0; s >>= 1) {
@@ -52,26 +83,35 @@ __device__ __forceinline__ double block_sum(double v, double *sh)
 }
 
 // PASS 0: partial sums of c and fluid-cell counts;  PASS 1: partial sums of (c - mean)^2, mean = res[0].
-// Block b handles box cells b*chunk .. (b+1)*chunk-1 (x fastest inside the box); part[b], part[G + b].
+// The box is walked by rows (j, k): block b takes rows b*rpb .. (b+1)*rpb-1, its warps take them in turn, the lanes
+// stride along x -- no division per cell, coalesced 256-byte reads.  part[b], part[G + b].
 template <int PASS>
-__global__ void __launch_bounds__(256) k_box_partial(const BoxArgs a, size_t chunk, const double *__restrict__ res, double *__restrict__ part)
+__global__ void __launch_bounds__(256) k_box_partial(const BoxArgs a, unsigned rows, unsigned rpb, const double *__restrict__ res,
+                                                     double *__restrict__ part)
 {
     __shared__ double sh[8];
     const double mean = PASS == 1 ? res[0] : 0.0;
-    const size_t beg = (size_t)blockIdx.x * chunk, end = beg + chunk < a.count ? beg + chunk : a.count;
+    const unsigned beg = blockIdx.x * rpb, end = beg + rpb < rows ? beg + rpb : rows;
+    const int lane = threadIdx.x & 31, wv = threadIdx.x >> 5;
     double s = 0.0, cnt = 0.0;
-    for (size_t n = beg + threadIdx.x; n < end; n += blockDim.x) {
-        const int i = (int)(n % a.size[0]), j = (int)((n / a.size[0]) % a.size[1]), k = (int)(n / ((size_t)a.size[0] * a.size[1]));
-        const size_t o = (size_t)((a.lo[0] + i) & (a.nx - 1)) +
-                         (size_t)a.nx * ((size_t)((a.lo[1] + j) & (a.ny - 1)) + (size_t)a.ny * ((a.lo[2] + k) & (a.nz - 1)));
-        if (a.face != nullptr && !(a.face[o] & 1)) continue;
-        const double cv = a.c[o];
-        if (PASS == 0) {
-            s += cv;
-            cnt += 1.0;
-        } else {
-            const double dv = cv - mean;
-            s += dv * dv;
+    for (unsigned row = beg + wv; row < end; row += 8) {
+        const unsigned k = row / (unsigned)a.size[1], j = row - k * (unsigned)a.size[1];
+        const size_t rowo = (size_t)a.nx * ((size_t)((a.lo[1] + j) & (a.ny - 1)) + (size_t)a.ny * ((a.lo[2] + k) & (a.nz - 1)));
+        const double *cr = a.c + rowo;
+        const uint8_t *fr = a.face != nullptr ? a.face + rowo : nullptr;
+        // four independent loads in flight per lane; solid cells add +0.0 (the sums keep their order)
+#pragma unroll 4
+        for (int i = lane; i < a.size[0]; i += 32) {
+            const int x = (a.lo[0] + i) & (a.nx - 1);
+            const bool fluid = fr == nullptr || (fr[x] & 1);
+            const double cv = __ldg(cr + x);
+            if (PASS == 0) {
+                s += fluid ? cv : 0.0;
+                cnt += fluid ? 1.0 : 0.0;
+            } else {
+                const double dv = cv - mean;
+                s += fluid ? dv * dv : 0.0;
+            }
         }
     }
     const double ts = block_sum(s, sh);

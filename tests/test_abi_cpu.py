@@ -19,7 +19,7 @@ def L():
 
 def test_every_declared_symbol_is_exported(L):
     hdr = open(os.path.join(ROOT, "include", "dnslab.h")).read()
-    declared = set(re.findall(r"\b(dnslab_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(dnslab_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(binding.SYMBOLS)
     for name in declared:
         assert hasattr(L, name), name

@@ -91,6 +91,31 @@ def test_poisson_two_pass_shapes_match_oracle(shape):
     assert torch.equal(buf, p)
 
 
+@pytest.mark.parametrize("shape", [(8, 8, 8), (16, 32, 64), (32, 8, 16), (8, 64, 128), (64, 16, 256), (32, 128, 512)])
+def test_rfft3_real_to_complex_transform_matches_oracle(shape):
+    """dnslab_rfft3 / dnslab_irfft3: the real-to-complex transform on its own (north_star names one) against the oracle's
+    full complex transform of the same real array (its kx = 0..nx/2 half), and back: irfft3(rfft3(x)) = x, irfft3 of the
+    oracle's half spectrum = x."""
+    import torch
+    rng = np.random.default_rng(sum(shape) + 7)
+    x = rng.standard_normal(shape)
+    nz, ny, nx = shape
+    s = binding.Solver(shape, (0.1, 0.1, 0.1), 0.1, 0.1, 0.1)
+    xd = torch.from_numpy(x).cuda()
+    X = s.rfft3(xd)
+    back = s.irfft3(X)
+    s.synchronize()
+    fr, fi = dnsref.fft3(x, np.zeros(shape), -1)
+    ref = (fr + 1j * fi)[:, :, : nx // 2 + 1]
+    tol = 1e-14 * np.log2(nx * ny * nz)
+    assert np.abs(X.cpu().numpy() - ref).max() <= tol * np.abs(ref).max()
+    assert np.abs(back.cpu().numpy() - x).max() <= tol * np.abs(x).max()
+    assert torch.equal(xd, torch.from_numpy(x).cuda())                     # the input is not modified
+    back2 = s.irfft3(torch.from_numpy(np.ascontiguousarray(ref)).cuda())
+    assert np.abs(back2.cpu().numpy() - x).max() <= tol * np.abs(x).max()
+    s.close()
+
+
 def test_poisson_null_modes_and_manufactured():
     import torch
     shape, d = (16, 32, 64), (0.2, 0.3, 0.25)
