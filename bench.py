@@ -510,7 +510,7 @@ def main():
     ap.add_argument("--mode", default="step", choices=["step", "reductions", "particles"],
                     help="step: the headline line; reductions / particles: the NEXT-3 / NEXT-4 lines")
     ap.add_argument("--particles", type=int, default=1000000, help="--mode particles: how many")
-    ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r02_ncu_full_raw.csv"),
+    ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r02c_ncu_full_raw.csv"),
                     help="ncu --page raw --csv export of a --set full capture of this workload (roofline.traffic)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
