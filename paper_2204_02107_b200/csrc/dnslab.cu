@@ -391,16 +391,10 @@ int launch_fft_z_solve(dnslab *h, c2 *data)
 // A tile of the xy pass is 8192 complex numbers (NY1 = 8192 / (nx/2) whole rows, 144 KB of shared memory with padding);
 // the fused middle pass takes NY0 = ny / NY1 rows by all of z for XT adjacent kx, at most 8192 numbers again.
 // Shapes outside these limits (and masks that need the dense eq. 9 prologue) use the five single-axis passes.
-#ifndef DNSLAB_XY_TILE
-#define DNSLAB_XY_TILE 4096
-#endif
-#ifndef DNSLAB_YZ_TILE
-#define DNSLAB_YZ_TILE 8192
-#endif
-#ifndef DNSLAB_YZ_XTMIN
-#define DNSLAB_YZ_XTMIN 4
-#endif
-constexpr int XY_TILE = DNSLAB_XY_TILE, YZ_TILE = DNSLAB_YZ_TILE, YZ_XTMIN = DNSLAB_YZ_XTMIN;
+// Tile sizes (measured on 512x256x128): xy tiles of 4096 points let two blocks share an SM (52 us per
+// pass; 8192-point tiles, one block per SM: 76 us); the middle pass then has NY0 = 16 and takes 8192-point tiles with runs
+// of XT = 4 complex numbers (99 us; 4096-point tiles with XT = 2: 117 us).
+constexpr int XY_TILE = 4096, YZ_TILE = 8192, YZ_XTMIN = 4;
 constexpr int xy_rows(int mx) { return XY_TILE / mx < 16 ? 16 : XY_TILE / mx; } // rows of an xy tile: at least 16 (one radix-16 column butterfly)
 
 int fused_ny1(const dnslab_params_t *P)
