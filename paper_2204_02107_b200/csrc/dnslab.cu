@@ -126,6 +126,8 @@ struct dnslab {
     int yz_ahead; // the same for the fused middle pass
     int xy_ahead; // two-pass solve, xy passes: how many blocks ahead a block prefetches into L2 (blocks resident on the chip)
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
+    bool tma_ok; // tensor maps of the 16 RK field buffers are built (k_rk_march loads interior tiles by TMA)
+    CUtensorMap tmap[16];
     long long np;      // NEXT-4: attached particles (0: none); state is the caller's device array
     double *pstate, prho_f, pgrav[3];
     // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
@@ -235,12 +237,20 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
         const dim3 blk(32, dnsst::RKM_TY, 1);
         const dim3 grd(h->P.nx / dnsst::RKM_TX, h->P.ny / dnsst::RKM_TY, h->P.nz / h->rk_kc);
         const size_t smem = dnsst::RKM_SMEM;
+        // tensor maps of the stage field's four buffers (any of the 16 RK field buffers can hold it: Q rotates)
+        dnsst::RKMaps maps;
+        a.use_tma = h->tma_ok ? 1 : 0;
+        for (int m = 0; m < 4; ++m) {
+            const size_t idx = ((const char *)qs[m] - (h->ws + h->L.off_fields)) / h->L.field_bytes;
+            if (idx >= 16) a.use_tma = 0;
+            maps.m[m] = h->tmap[idx < 16 ? idx : 0];
+        }
 #define DNS_LAUNCH_MARCH(M, S)                                                                                          \
     do {                                                                                                                \
         auto kern = dnsst::k_rk_march<STAGE, ELIM, M, S>;                                                               \
         if (h->prepare) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess ? DNSLAB_OK : DNSLAB_ECUDA; \
         ProfScope ps(h, DNSLAB_K_RK);                                                                                   \
-        kern<<<grd, blk, smem, h->stream>>>(a);                                                                         \
+        kern<<<grd, blk, smem, h->stream>>>(a, maps);                                                                   \
     } while (0)
         if (masked && sources) DNS_LAUNCH_MARCH(true, true);
         else if (masked) DNS_LAUNCH_MARCH(true, false);
@@ -730,6 +740,32 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
             while (kc > 8 && tiles * (params->nz / kc) < 6L * 2 * prop.multiProcessorCount) kc /= 2;
             h->rk_kc = kc;
         }
+    }
+
+    // TMA descriptors for k_rk_march's plane tiles: rank 3 (x, y, z), fp64, box 68 x 10 x 1, out-of-bounds = zero (only
+    // interior blocks use them).  The encoder is a driver entry point fetched at run time; without it (or for the brick
+    // kernel of small grids) every block copies its tiles with cp.async.
+    h->tma_ok = false;
+    if (h->rk_kc > 0) {
+        typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                      const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                      CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void *fp = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qres) == cudaSuccess && fp != nullptr &&
+            qres == cudaDriverEntryPointSuccess) {
+            const cuuint64_t gdim[3] = {(cuuint64_t)params->nx, (cuuint64_t)params->ny, (cuuint64_t)params->nz};
+            const cuuint64_t gstr[2] = {(cuuint64_t)params->nx * sizeof(double), (cuuint64_t)params->nx * params->ny * sizeof(double)};
+            const cuuint32_t box[3] = {(cuuint32_t)dnsst::RKM_SW, (cuuint32_t)dnsst::RKM_ROWS, 1u};
+            const cuuint32_t estr[3] = {1u, 1u, 1u};
+            bool ok = true;
+            for (int b = 0; b < 16 && ok; ++b)
+                ok = ((encode_fn)fp)(&h->tmap[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)fld(b), gdim, gstr, box, estr,
+                                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+            h->tma_ok = ok;
+        }
+        (void)cudaGetLastError();
     }
 
     auto fail = [&](int rc) { delete h; return rc; };

@@ -2,6 +2,7 @@
 // fused RHS + Runge-Kutta stage update, divergence, pressure-gradient projection, mask set-up.
 // fp64, x fastest, all axes periodic with power-of-two extents (wrap = bit mask).
 #pragma once
+#include <cuda.h> // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint, nothing links libcuda)
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -68,6 +69,7 @@ struct RKArgs {
     int nsrc;
     int kc;                  // k_rk_march: planes per block
     int rev;                 // k_rk_march: walk the y tiles and z chunks from the far end (start on what the kernel before left in L2)
+    int use_tma;             // k_rk_march: tensor maps of the stage field are valid (interior blocks load their tiles by TMA)
     const double *stab;
     RhsCoef kf;
     SourceDev src[DNS_MAX_SRC];
@@ -189,7 +191,46 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
 // the other operands (Qn, Q2, Q3) and the result are streamed as 16-byte accesses.
 // One __syncthreads per plane.  Arithmetic and select semantics are those of k_rk above.
 constexpr int RKM_TX = 64, RKM_TY = 8, RKM_SW = 68, RKM_ROWS = RKM_TY + 2, RKM_NBUF = 4; // 5 tiles (three planes in flight) measured slower: 1.31 vs 1.10 ms per step
-constexpr int RKM_SMEM = RKM_NBUF * 4 * RKM_ROWS * RKM_SW * (int)sizeof(double);
+constexpr int RKM_FS = 688;                                      // doubles per field tile: 10 x 68 = 680, padded to a multiple of 128 bytes (TMA destination)
+constexpr int RKM_TILE_BYTES = RKM_ROWS * RKM_SW * (int)sizeof(double); // what one TMA box writes
+constexpr int RKM_SMEM = RKM_NBUF * 4 * RKM_FS * (int)sizeof(double);
+
+// The four tensor maps of a stage field (one per component): rank 3 (x, y, z), fp64, box 68 x 10 x 1.
+struct RKMaps {
+    CUtensorMap m[4];
+};
+
+// ---- mbarrier / TMA (cp.async.bulk.tensor) in raw PTX ---------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    asm volatile("{\n"
+                 ".reg .pred p;\n"
+                 "MBAR_WAIT_%=:\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                 "@p bra MBAR_DONE_%=;\n"
+                 "bra MBAR_WAIT_%=;\n"
+                 "MBAR_DONE_%=:\n"
+                 "}\n" ::"r"(smem_u32(bar)),
+                 "r"(parity)
+                 : "memory");
+}
+// one box of a rank-3 tensor map into shared memory (128-byte aligned); completion is counted in bytes on `bar`
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];\n" ::"r"(smem_u32(dst)),
+                 "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
+}
 
 __device__ __forceinline__ void cp_async16(void *dst_smem, const void *src)
 {
@@ -230,10 +271,12 @@ __device__ __forceinline__ double rk_rhs_cell(const RKArgs &a, int m, unsigned f
     return val;
 }
 
-template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __launch_bounds__(256, 2) k_rk_march(const RKArgs a)
+template <int STAGE, bool ELIM, bool MASKED, bool SOURCES>
+__global__ void __launch_bounds__(256, 2) k_rk_march(const RKArgs a, const __grid_constant__ RKMaps maps)
 {
-    constexpr int TX = RKM_TX, SW = RKM_SW, ROWS = RKM_ROWS, PLANE = 4 * RKM_ROWS * RKM_SW;
-    extern __shared__ double2 rkm_smem2[];
+    constexpr int TX = RKM_TX, SW = RKM_SW, ROWS = RKM_ROWS, FS = RKM_FS, PLANE = 4 * RKM_FS;
+    extern __shared__ __align__(128) double2 rkm_smem2[];
+    __shared__ __align__(8) uint64_t mbar[RKM_NBUF];
     double *sm = reinterpret_cast<double *>(rkm_smem2);
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * 32 + tx;
     const int nx = a.nx, ny = a.ny, nz = a.nz, kc = a.kc;
@@ -254,17 +297,36 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
     const bool has_h = tid >= 64 && tid < 64 + 4 * ROWS * 2;  // x halo: 80 values
     const int hh = tid - 64, h_m = hh / (ROWS * 2), h_r = (hh % (ROWS * 2)) >> 1, h_s = hh & 1;
     const unsigned src_h = (unsigned)nx * ((y0 - 1 + h_r) & (ny - 1)) + (h_s ? ((x0 + TX) & (nx - 1)) : ((x0 - 1) & (nx - 1)));
-    const int dst_h = (h_m * ROWS + h_r) * SW + (h_s ? 2 + TX : 1);
+    const int dst_h = h_m * FS + h_r * SW + (h_s ? 2 + TX : 1);
     const double *qs_h = has_h ? a.qs[h_m & 3] : a.qs[0];
-    auto issue_plane = [&](int kk, int buf) {
-        const unsigned pk = plane * (unsigned)(kk & (nz - 1));
-        double *sb = sm + buf * PLANE;
+    // Interior blocks (the 68 x 10 box x0-2 .. x0+65, y0-1 .. y0+8 lies inside the grid: 70 % of the blocks of a
+    // 512 x 256 plane) fetch a plane tile with four TMA box loads issued by one thread, counted in bytes on the tile's
+    // mbarrier; blocks at the periodic seams, where a box would be zero-filled instead of wrapped, copy their tiles
+    // with per-thread cp.async whose source addresses wrap.  Same tile layout for both.
+    const bool tma = a.use_tma && blockIdx.x >= 1 && blockIdx.x + 2 <= gridDim.x && by >= 1 && by + 2 <= (int)gridDim.y;
+    if (tma && tid == 0) {
 #pragma unroll
-        for (int m = 0; m < 4; ++m) {
-            cp_async16(sb + m * ROWS * SW + dst_a, a.qs[m] + (pk + src_a));
-            if (has_b) cp_async16(sb + m * ROWS * SW + dst_b, a.qs[m] + (pk + src_b));
+        for (int b = 0; b < RKM_NBUF; ++b) mbar_init(&mbar[b], 1);
+        mbar_fence_init();
+    }
+    if (tma) __syncthreads();
+    auto issue_plane = [&](int kk, int buf) {
+        double *sb = sm + buf * PLANE;
+        if (tma) {
+            if (tid == 0) {
+                mbar_arrive_expect_tx(&mbar[buf], 4 * RKM_TILE_BYTES);
+#pragma unroll
+                for (int m = 0; m < 4; ++m) tma_load_3d(sb + m * FS, &maps.m[m], &mbar[buf], x0 - 2, y0 - 1, kk & (nz - 1));
+            }
+        } else {
+            const unsigned pk = plane * (unsigned)(kk & (nz - 1));
+#pragma unroll
+            for (int m = 0; m < 4; ++m) {
+                cp_async16(sb + m * FS + dst_a, a.qs[m] + (pk + src_a));
+                if (has_b) cp_async16(sb + m * FS + dst_b, a.qs[m] + (pk + src_b));
+            }
+            if (has_h) cp_async8(sb + dst_h, qs_h + (pk + src_h));
         }
-        if (has_h) cp_async8(sb + dst_h, qs_h + (pk + src_h));
         cp_async_commit();
     };
 
@@ -309,16 +371,20 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
             if (STAGE == 4 && ELIM) q2[m] = *reinterpret_cast<const double2 *>(a.qc[m] + o);  // S, overwritten below by Q*
         }
         cp_async_wait_n<RKM_NBUF - 3>();
+        if (tma) { // the tile of plane k+1 (and of plane k at the first step) has landed: tile n of the block is use n/4 of its mbarrier
+            if (t == 0) mbar_wait(&mbar[0], 0);
+            mbar_wait(&mbar[(t + 1) % RKM_NBUF], ((t + 1) / RKM_NBUF) & 1);
+        }
         __syncthreads(); // plane k+1 visible to all; every thread is done with the tile of plane k-1
         if (t + RKM_NBUF - 1 <= kc) issue_plane(k + RKM_NBUF - 1, (t + RKM_NBUF - 1) % RKM_NBUF);
         else cp_async_commit();
         const double *sC = sm + (t % RKM_NBUF) * PLANE, *sN = sm + ((t + 1) % RKM_NBUF) * PLANE;
         if (t == 0) {
 #pragma unroll
-            for (int m = 0; m < 4; ++m) cur[m] = *reinterpret_cast<const double2 *>(sC + m * ROWS * SW + own);
+            for (int m = 0; m < 4; ++m) cur[m] = *reinterpret_cast<const double2 *>(sC + m * FS + own);
         }
 #pragma unroll
-        for (int m = 0; m < 4; ++m) zp[m] = *reinterpret_cast<const double2 *>(sN + m * ROWS * SW + own);
+        for (int m = 0; m < 4; ++m) zp[m] = *reinterpret_cast<const double2 *>(sN + m * FS + own);
         if (STAGE == 1) {
 #pragma unroll
             for (int m = 0; m < 4; ++m) qn[m] = cur[m];
@@ -327,8 +393,8 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
         //   A+-_a = -(u_a(+-a) + u_a)/(4 Delta_a), then F = sum_a [q(+a)(A+_a + D_a) + q(-a)(D_a - A-_a)] - 2 sum_a D_a q0 + b
         double axp[2], axm[2], ayp[2], aym[2], azp[2], azm[2];
         {
-            const double2 vym = *reinterpret_cast<const double2 *>(sC + 1 * ROWS * SW + own - SW);
-            const double2 vyp = *reinterpret_cast<const double2 *>(sC + 1 * ROWS * SW + own + SW);
+            const double2 vym = *reinterpret_cast<const double2 *>(sC + 1 * FS + own - SW);
+            const double2 vyp = *reinterpret_cast<const double2 *>(sC + 1 * FS + own + SW);
             const double uxmA = sC[own - 1], uxpB = sC[own + 2];
             axp[0] = (cur[0].y + cur[0].x) * kf.hx; axm[0] = (uxmA + cur[0].x) * kf.hx;
             axp[1] = (uxpB + cur[0].y) * kf.hx;     axm[1] = axp[0];
@@ -347,7 +413,7 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
             double2 F[4];
             {
                 // scalar first: its diffusive coefficients carry the face bits of eq. 4
-                const double *sf = sC + 3 * ROWS * SW + own;
+                const double *sf = sC + 3 * FS + own;
                 const double2 ym = *reinterpret_cast<const double2 *>(sf - SW), yp = *reinterpret_cast<const double2 *>(sf + SW);
                 const double xpv[2] = {cur[3].y, sf[2]}, xmv[2] = {sf[-1], cur[3].x};
                 const double ypv[2] = {yp.x, yp.y}, ymv[2] = {ym.x, ym.y}, zpv[2] = {zp[3].x, zp[3].y}, zmv[2] = {zm[3].x, zm[3].y};
@@ -391,7 +457,7 @@ template <int STAGE, bool ELIM, bool MASKED, bool SOURCES> __global__ void __lau
             }
 #pragma unroll
             for (int m = 0; m < 3; ++m) {
-                const double *sf = sC + m * ROWS * SW + own;
+                const double *sf = sC + m * FS + own;
                 const double2 ym = *reinterpret_cast<const double2 *>(sf - SW), yp = *reinterpret_cast<const double2 *>(sf + SW);
                 const double xmA = sf[-1], xpB = sf[2];
                 double vx = fma(kf.dv0, cur[m].x, a.body[m]), vy = fma(kf.dv0, cur[m].y, a.body[m]);
