@@ -5,7 +5,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "dnslab.cu")
-DEPS = [SRC, os.path.join(HERE, "csrc", "fft.cuh"), os.path.join(HERE, "csrc", "stencil.cuh"), os.path.join(HERE, "csrc", "reduce.cuh"), os.path.join(HERE, "csrc", "particles.cuh"),
+DEPS = [SRC, os.path.join(HERE, "csrc", "fft.cuh"), os.path.join(HERE, "csrc", "stencil.cuh"), os.path.join(HERE, "csrc", "reduce.cuh"), os.path.join(HERE, "csrc", "particles.cuh"), os.path.join(HERE, "csrc", "tma.cuh"),
         os.path.join(os.path.dirname(HERE), "include", "dnslab.h")]
 LIB = os.path.join(HERE, "libdnslab.so")
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -128,6 +128,9 @@ struct dnslab {
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
     bool tma_ok; // tensor maps of the 16 RK field buffers are built (k_rk_march loads interior tiles by TMA)
     CUtensorMap tmap[16];
+    void *tma_encode; // cuTensorMapEncodeTiled, fetched through cudaGetDriverEntryPoint at create (null: no TMA anywhere)
+    bool wmap_ok;     // the tensor map of the transform array W is built: the middle pass of the two-pass solve moves its tile by TMA
+    CUtensorMap wmap;
     long long np;      // NEXT-4: attached particles (0: none); state is the caller's device array
     double *pstate, prho_f, pgrav[3];
     // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
@@ -196,6 +199,20 @@ dim3 tile_block(const dnslab *h)
     int by = 256 / bx;
     if (by > h->P.ny) by = h->P.ny;
     return dim3(bx, by, 1);
+}
+
+// One rank-3 fp64 tensor map (x fastest) through the driver entry point fetched at create; false when it is unavailable.
+bool encode_map3(dnslab *h, CUtensorMap *map, void *base, const cuuint64_t (&gdim)[3], const cuuint32_t (&box)[3],
+                 CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_128B)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    if (!h->tma_encode) return false;
+    const cuuint64_t gstr[2] = {gdim[0] * sizeof(double), gdim[0] * gdim[1] * sizeof(double)};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    return ((encode_fn)h->tma_encode)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                      CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // ---- RK stage ---------------------------------------------------------------------------
@@ -447,11 +464,39 @@ template <int DIR> int launch_fft_xy(dnslab *h, const c2 *in, c2 *out)
     return DNSLAB_EINVAL;
 }
 
+// Middle pass with its tile moved by TMA (k_fft_zy_solve_tma): tiles of YZ_TMA_TILE points, runs of at least 2 complex numbers.
+#ifndef DNSLAB_YZ_PROMO
+#define DNSLAB_YZ_PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+#endif
+#ifndef DNSLAB_YZ_TMA_TILE
+#define DNSLAB_YZ_TMA_TILE 4096
+#endif
+constexpr int YZ_TMA_TILE = DNSLAB_YZ_TMA_TILE; // 0: the kernel with ordinary loads and stores
+
 template <int NY0, int LZ> int launch_fft_yz_solve_NL(dnslab *h, c2 *data)
 {
+    const int mx = h->P.nx / 2;
+    if constexpr (YZ_TMA_TILE > 0) {
+        constexpr int XT = (YZ_TMA_TILE / (NY0 * LZ)) > 16 ? 16 : ((YZ_TMA_TILE / (NY0 * LZ)) < 2 ? 2 : YZ_TMA_TILE / (NY0 * LZ));
+        constexpr int NT = XT * NY0 * LZ / 16, ZB = LZ > 256 ? 256 : LZ;
+        const size_t smem = (size_t)LZ * (NY0 * XT + (XT < 8 ? XT : 0)) * sizeof(c2) + LZ * (sizeof(c2) + sizeof(double)) + NY0 * sizeof(double);
+        auto kern = dnsfft::k_fft_zy_solve_tma<NY0, LZ, XT>;
+        if (h->prepare) {
+            const cuuint64_t gdim[3] = {(cuuint64_t)(2 * mx), (cuuint64_t)h->P.ny, (cuuint64_t)h->P.nz};
+            const cuuint32_t box[3] = {(cuuint32_t)(2 * XT), (cuuint32_t)NY0, (cuuint32_t)ZB};
+            h->wmap_ok = data == reinterpret_cast<c2 *>(h->W) && encode_map3(h, &h->wmap, (void *)data, gdim, box, (CUtensorMapL2promotion)DNSLAB_YZ_PROMO);
+            if (h->wmap_ok && smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        }
+        if (h->wmap_ok && data == reinterpret_cast<c2 *>(h->W)) {
+            if (h->prepare) return DNSLAB_OK;
+            ProfScope ps(h, DNSLAB_K_FFT_YZ);
+            kern<<<(unsigned)((mx / XT) * (h->P.ny / NY0)), NT, smem, h->stream>>>(h->wmap, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2],
+                                                                                  2.0 / (double)h->n, 1);
+            return check_launch(h);
+        }
+    }
     constexpr int XT = (YZ_TILE / (NY0 * LZ)) > 16 ? 16 : ((YZ_TILE / (NY0 * LZ)) < 1 ? 1 : YZ_TILE / (NY0 * LZ)), NT = XT * NY0 * LZ / 16;
     const size_t smem = (size_t)LZ * (NY0 * XT + (XT < 8 ? XT : 0)) * sizeof(c2) + LZ * (sizeof(c2) + sizeof(double));
-    const int mx = h->P.nx / 2;
     auto kern = dnsfft::k_fft_yz_solve<NY0, LZ, XT>;
     if (h->prepare) {
         if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -746,26 +791,22 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
     // interior blocks use them).  The encoder is a driver entry point fetched at run time; without it (or for the brick
     // kernel of small grids) every block copies its tiles with cp.async.
     h->tma_ok = false;
-    if (h->rk_kc > 0) {
-        typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
-                                      const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                      CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    h->wmap_ok = false;
+    h->tma_encode = nullptr;
+    {
         void *fp = nullptr;
         cudaDriverEntryPointQueryResult qres;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qres) == cudaSuccess && fp != nullptr &&
-            qres == cudaDriverEntryPointSuccess) {
-            const cuuint64_t gdim[3] = {(cuuint64_t)params->nx, (cuuint64_t)params->ny, (cuuint64_t)params->nz};
-            const cuuint64_t gstr[2] = {(cuuint64_t)params->nx * sizeof(double), (cuuint64_t)params->nx * params->ny * sizeof(double)};
-            const cuuint32_t box[3] = {(cuuint32_t)dnsst::RKM_SW, (cuuint32_t)dnsst::RKM_ROWS, 1u};
-            const cuuint32_t estr[3] = {1u, 1u, 1u};
-            bool ok = true;
-            for (int b = 0; b < 16 && ok; ++b)
-                ok = ((encode_fn)fp)(&h->tmap[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)fld(b), gdim, gstr, box, estr,
-                                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-            h->tma_ok = ok;
-        }
+            qres == cudaDriverEntryPointSuccess)
+            h->tma_encode = fp;
         (void)cudaGetLastError();
+    }
+    if (h->rk_kc > 0) {
+        const cuuint64_t gdim[3] = {(cuuint64_t)params->nx, (cuuint64_t)params->ny, (cuuint64_t)params->nz};
+        const cuuint32_t box[3] = {(cuuint32_t)dnsst::RKM_SW, (cuuint32_t)dnsst::RKM_ROWS, 1u};
+        bool ok = true;
+        for (int b = 0; b < 16 && ok; ++b) ok = encode_map3(h, &h->tmap[b], (void *)fld(b), gdim, box);
+        h->tma_ok = ok;
     }
 
     auto fail = [&](int rc) { delete h; return rc; };

@@ -14,6 +14,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "tma.cuh"
+
 namespace dnsfft {
 
 typedef double2 c2;
@@ -617,6 +619,105 @@ __global__ void __launch_bounds__(XT *NY0 *LZ / 16, (XT * NY0 * LZ / 16 <= 256 ?
     for (int g = 0; g < G; ++g)
 #pragma unroll
         for (int y0 = 0; y0 < NY0; ++y0) g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx] = x[g * NY0 + y0];
+}
+
+// k_fft_zy_solve_tma: the same middle pass with its tile moved by TMA.  The complex array is a rank-3 tensor
+// (2 mx doubles, ny, nz); one box (2 XT, NY0, LZ) is the whole tile, landing dense as [z][y0][xl].  A dense tile is
+// conflict-free for threads that hold a z line (lanes on adjacent (xl, y0)), so z is transformed FIRST here, straight out
+// of the landing buffer, and y0 second (through the padded layout of the kernel above); the result goes back the same way
+// and leaves by one TMA store.  No load or store instruction touches global memory, no register waits on one: runs of
+// XT = 2 numbers (32 bytes) cost the LSU nothing, so tiles of 4096 points -- two blocks per SM -- become affordable.
+template <int NY0, int LZ, int XT>
+__global__ void __launch_bounds__(XT *NY0 *LZ / 16, (XT * NY0 * LZ / 16 <= 256 ? 2 : 1))
+    k_fft_zy_solve_tma(const __grid_constant__ CUtensorMap map, const c2 *__restrict__ twz, int mx, int ny, const double *__restrict__ ex,
+                       const double *__restrict__ ey, const double *__restrict__ ez, double inv_n, int rev)
+{
+    using namespace dnstma;
+    constexpr int E = 16, G = E / NY0, ZQ = LZ / G, T = LZ / E, NT = XT * NY0 * LZ / E;
+    constexpr int DROW = NY0 * XT;                     // one z plane of the dense (TMA) layout
+    constexpr int ZROW = NY0 * XT + (XT < 8 ? XT : 0); // and of the padded layout between the z and the y0 transform
+    constexpr int ZB = LZ > 256 ? 256 : LZ;            // planes per box (a box extent is at most 256)
+    static_assert(NY0 >= 2 && NY0 <= 16 && LZ >= 32, "unsupported split");
+    extern __shared__ __align__(128) double2 smem[];
+    __shared__ __align__(8) uint64_t mbar;
+    c2 *stw = smem + LZ * ZROW;                         // z twiddles exp(-2 pi i t/LZ)
+    double *sez = reinterpret_cast<double *>(stw + LZ); // z eigenvalue parts
+    double *sey = sez + LZ;                             // y eigenvalue parts of this block's NY0 frequencies ky1 + ny1 ky0
+    const int ny1 = ny / NY0, xtiles = mx / XT;
+    const unsigned bid = rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const int xt = bid % xtiles, ky1 = bid / xtiles;
+    const int t = threadIdx.x, xl = t % XT, rest = t / XT;
+    const int y0 = rest % NY0, tid = rest / NY0; // z layout: planes tid + e T of one (xl, y0)
+    const int zq = rest;                         // y0 layout: all NY0 values of the planes zq + g ZQ
+    if (t == 0) {
+        mbar_init(&mbar, 1);
+        mbar_fence_init();
+        mbar_arrive_expect_tx(&mbar, (unsigned)(LZ * DROW * sizeof(c2)));
+#pragma unroll
+        for (int z0 = 0; z0 < LZ; z0 += ZB) tma_load_3d(smem + z0 * DROW, &map, &mbar, 2 * xt * XT, ky1 * NY0, z0);
+    }
+    for (int q = t; q < LZ; q += NT) {
+        sez[q] = ez[q];
+        stw[q] = twz[q];
+    }
+    if (t < NY0) sey[t] = ey[ky1 + ny1 * t];
+    __syncthreads(); // tables, and the initialised barrier, are visible to every thread
+    mbar_wait(&mbar, 0);
+    SmStride<DROW> sd{smem + y0 * XT + xl};
+    c2 x[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) x[e] = sd.at(tid + e * T);
+    __syncthreads();
+    fft_line<LZ, E, -1, 1, SmStride<DROW>>(x, tid, stw, sd);
+#pragma unroll
+    for (int e = 0; e < E; ++e) smem[(tid + e * T) * ZROW + y0 * XT + xl] = x[e];
+    __syncthreads();
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = smem[(zq + g * ZQ) * ZROW + q * XT + xl];
+#pragma unroll
+    for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
+    {
+        const int m = xt * XT + xl;
+        const double exm = __ldg(&ex[m]);
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const int kz = zq + g * ZQ;
+            const double exz = exm + sez[kz];
+            const bool null_xz = (m == 0) && (((2 * kz) & (LZ - 1)) == 0);
+#pragma unroll
+            for (int q = 0; q < NY0; ++q) {
+                const int ky = ky1 + ny1 * q;
+                const double lam = -(exz + sey[q]);
+                const bool null = null_xz && (((2 * ky) & (ny - 1)) == 0);
+                const double sc = inv_n * rcp_newton(lam);
+                x[g * NY0 + q].x = null ? 0.0 : x[g * NY0 + q].x * sc;
+                x[g * NY0 + q].y = null ? 0.0 : x[g * NY0 + q].y * sc;
+            }
+        }
+    }
+#pragma unroll
+    for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int q = 0; q < NY0; ++q) smem[(zq + g * ZQ) * ZROW + q * XT + xl] = x[g * NY0 + q];
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < E; ++e) x[e] = smem[(tid + e * T) * ZROW + y0 * XT + xl];
+    __syncthreads();
+    fft_line<LZ, E, +1, 1, SmStride<DROW>>(x, tid, stw, sd);
+#pragma unroll
+    for (int e = 0; e < E; ++e) sd.at(tid + e * T) = x[e];
+    fence_proxy_async();
+    __syncthreads();
+    if (t == 0) {
+#pragma unroll
+        for (int z0 = 0; z0 < LZ; z0 += ZB) tma_store_3d(&map, smem + z0 * DROW, 2 * xt * XT, ky1 * NY0, z0);
+        tma_store_commit();
+        tma_store_wait_read();
+    }
 }
 
 // ---------------------------------------------------------------------------------------

@@ -6,7 +6,11 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "tma.cuh"
+
 namespace dnsst {
+
+using namespace dnstma;
 
 #define DNS_MAX_SRC 16
 
@@ -199,38 +203,6 @@ constexpr int RKM_SMEM = RKM_NBUF * 4 * RKM_FS * (int)sizeof(double);
 struct RKMaps {
     CUtensorMap m[4];
 };
-
-// ---- mbarrier / TMA (cp.async.bulk.tensor) in raw PTX ---------------------------------------------------------------
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
-{
-    asm volatile("{\n"
-                 ".reg .pred p;\n"
-                 "MBAR_WAIT_%=:\n"
-                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-                 "@p bra MBAR_DONE_%=;\n"
-                 "bra MBAR_WAIT_%=;\n"
-                 "MBAR_DONE_%=:\n"
-                 "}\n" ::"r"(smem_u32(bar)),
-                 "r"(parity)
-                 : "memory");
-}
-// one box of a rank-3 tensor map into shared memory (128-byte aligned); completion is counted in bytes on `bar`
-__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2)
-{
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];\n" ::"r"(smem_u32(dst)),
-                 "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
-                 : "memory");
-}
 
 __device__ __forceinline__ void cp_async16(void *dst_smem, const void *src)
 {
