@@ -123,13 +123,12 @@ struct dnslab {
     int nsm;   // SM count of the device
     bool prepare; // set while dnslab_create walks the launchers once: they configure their kernel and do not launch
     unsigned zgrid; // grid of the persistent fused middle pass (occupancy query done once, at create)
-    int yz_ahead; // the same for the fused middle pass
     int xy_ahead; // two-pass solve, xy passes: how many blocks ahead a block prefetches into L2 (blocks resident on the chip)
     int rk_kc; // > 0: z-marching RK kernel with this many planes per block; 0: brick kernel (small grids)
     bool tma_ok; // tensor maps of the 16 RK field buffers are built (k_rk_march loads interior tiles by TMA)
     CUtensorMap tmap[16];
     void *tma_encode; // cuTensorMapEncodeTiled, fetched through cudaGetDriverEntryPoint at create (null: no TMA anywhere)
-    bool wmap_ok;     // the tensor map of the transform array W is built: the middle pass of the two-pass solve moves its tile by TMA
+    bool wmap_ok;     // the tensor map of the transform array W is built (the middle pass of the two-pass solve moves its tiles by TMA)
     CUtensorMap wmap;
     long long np;      // NEXT-4: attached particles (0: none); state is the caller's device array
     double *pstate, prho_f, pgrav[3];
@@ -415,13 +414,14 @@ int launch_fft_z_solve(dnslab *h, c2 *data)
 }
 
 // ---- two-pass solve: k_fft_xy (x and the high digit of y) and k_fft_yz_solve (low digit of y, z, division) --------
-// A tile of the xy pass is 8192 complex numbers (NY1 = 8192 / (nx/2) whole rows, 144 KB of shared memory with padding);
-// the fused middle pass takes NY0 = ny / NY1 rows by all of z for XT adjacent kx, at most 8192 numbers again.
+// A tile of the xy pass is 4096 complex numbers (NY1 = 4096 / (nx/2) whole rows, at least 16; 70 KB of shared memory with
+// padding, two blocks per SM); the fused middle pass takes NY0 = ny / NY1 rows by all of z for XT adjacent kx, 4096 numbers
+// again, with runs of at least XT = 2 complex numbers (its tiles move by TMA, so short runs cost no LSU instructions).
 // Shapes outside these limits (and masks that need the dense eq. 9 prologue) use the five single-axis passes.
-// Tile sizes (measured on 512x256x128): xy tiles of 4096 points let two blocks share an SM (52 us per
-// pass; 8192-point tiles, one block per SM: 76 us); the middle pass then has NY0 = 16 and takes 8192-point tiles with runs
-// of XT = 4 complex numbers (99 us; 4096-point tiles with XT = 2: 117 us).
-constexpr int XY_TILE = 4096, YZ_TILE = 8192, YZ_XTMIN = 4;
+// Measured on 512x256x128: xy tiles of 8192 points, one block per SM: 76 instead of 51 us per pass;
+// middle pass with ordinary loads and stores: 99 us (8192 points, XT = 4) / 117 us (4096 points, XT = 2); by TMA: 113 us
+// (8192 points, one block per SM), 80 us (4096 points, two blocks per SM), 76 us (4096 points, persistent two-group blocks).
+constexpr int XY_TILE = 4096, YZ_TILE = 4096, YZ_XTMIN = 2;
 constexpr int xy_rows(int mx) { return XY_TILE / mx < 16 ? 16 : XY_TILE / mx; } // rows of an xy tile: at least 16 (one radix-16 column butterfly)
 
 int fused_ny1(const dnslab_params_t *P)
@@ -464,50 +464,31 @@ template <int DIR> int launch_fft_xy(dnslab *h, const c2 *in, c2 *out)
     return DNSLAB_EINVAL;
 }
 
-// Middle pass with its tile moved by TMA (k_fft_zy_solve_tma): tiles of YZ_TMA_TILE points, runs of at least 2 complex numbers.
-#ifndef DNSLAB_YZ_PROMO
-#define DNSLAB_YZ_PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_128B
-#endif
-#ifndef DNSLAB_YZ_TMA_TILE
-#define DNSLAB_YZ_TMA_TILE 4096
-#endif
-constexpr int YZ_TMA_TILE = DNSLAB_YZ_TMA_TILE; // 0: the kernel with ordinary loads and stores
-
+// Middle pass (k_fft_yz_solve): persistent blocks of two groups, tiles of YZ_TILE points moved by TMA -- one landing buffer,
+// two work buffers and the z tables in shared memory (207 KB on 512x256x128).
 template <int NY0, int LZ> int launch_fft_yz_solve_NL(dnslab *h, c2 *data)
 {
+    constexpr int XT = (YZ_TILE / (NY0 * LZ)) > 16 ? 16 : YZ_TILE / (NY0 * LZ);
+    static_assert(XT >= YZ_XTMIN, "tile too large");
+    constexpr int NT = XT * NY0 * LZ / 16, ZB = LZ > 256 ? 256 : LZ;
     const int mx = h->P.nx / 2;
-    if constexpr (YZ_TMA_TILE > 0) {
-        constexpr int XT = (YZ_TMA_TILE / (NY0 * LZ)) > 16 ? 16 : ((YZ_TMA_TILE / (NY0 * LZ)) < 2 ? 2 : YZ_TMA_TILE / (NY0 * LZ));
-        constexpr int NT = XT * NY0 * LZ / 16, ZB = LZ > 256 ? 256 : LZ;
-        const size_t smem = (size_t)LZ * (NY0 * XT + (XT < 8 ? XT : 0)) * sizeof(c2) + LZ * (sizeof(c2) + sizeof(double)) + NY0 * sizeof(double);
-        auto kern = dnsfft::k_fft_zy_solve_tma<NY0, LZ, XT>;
-        if (h->prepare) {
-            const cuuint64_t gdim[3] = {(cuuint64_t)(2 * mx), (cuuint64_t)h->P.ny, (cuuint64_t)h->P.nz};
-            const cuuint32_t box[3] = {(cuuint32_t)(2 * XT), (cuuint32_t)NY0, (cuuint32_t)ZB};
-            h->wmap_ok = data == reinterpret_cast<c2 *>(h->W) && encode_map3(h, &h->wmap, (void *)data, gdim, box, (CUtensorMapL2promotion)DNSLAB_YZ_PROMO);
-            if (h->wmap_ok && smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        }
-        if (h->wmap_ok && data == reinterpret_cast<c2 *>(h->W)) {
-            if (h->prepare) return DNSLAB_OK;
-            ProfScope ps(h, DNSLAB_K_FFT_YZ);
-            kern<<<(unsigned)((mx / XT) * (h->P.ny / NY0)), NT, smem, h->stream>>>(h->wmap, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2],
-                                                                                  2.0 / (double)h->n, 1);
-            return check_launch(h);
-        }
-    }
-    constexpr int XT = (YZ_TILE / (NY0 * LZ)) > 16 ? 16 : ((YZ_TILE / (NY0 * LZ)) < 1 ? 1 : YZ_TILE / (NY0 * LZ)), NT = XT * NY0 * LZ / 16;
-    const size_t smem = (size_t)LZ * (NY0 * XT + (XT < 8 ? XT : 0)) * sizeof(c2) + LZ * (sizeof(c2) + sizeof(double));
+    const size_t smem = dnsfft::YzLayout<NY0, LZ, XT>::SMEM;
+    static_assert(dnsfft::YzLayout<NY0, LZ, XT>::SMEM <= 227 * 1024, "middle-pass buffers exceed the shared memory of an SM");
     auto kern = dnsfft::k_fft_yz_solve<NY0, LZ, XT>;
     if (h->prepare) {
-        if (smem > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int per_sm = 0;
-        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
-        h->yz_ahead = per_sm * h->nsm;
+        // the transform array as a rank-3 tensor of doubles (2 mx, ny, nz); one box is a tile (at most 256 planes per box)
+        const cuuint64_t gdim[3] = {(cuuint64_t)(2 * mx), (cuuint64_t)h->P.ny, (cuuint64_t)h->P.nz};
+        const cuuint32_t box[3] = {(cuuint32_t)(2 * XT), (cuuint32_t)NY0, (cuuint32_t)ZB};
+        h->wmap_ok = encode_map3(h, &h->wmap, (void *)data, gdim, box);
+        if (h->wmap_ok) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         return DNSLAB_OK;
     }
+    const size_t ntiles = (size_t)(mx / XT) * (h->P.ny / NY0);
+    size_t g = (size_t)h->nsm < ntiles ? (size_t)h->nsm : ntiles;
+    const size_t per_block = (ntiles + g - 1) / g; // equal shares: the smallest grid that needs the same number of tiles per block
+    g = (ntiles + per_block - 1) / per_block;
     ProfScope ps(h, DNSLAB_K_FFT_YZ);
-    kern<<<(unsigned)((mx / XT) * (h->P.ny / NY0)), NT, smem, h->stream>>>(data, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2],
-                                                                          2.0 / (double)h->n, 1, h->yz_ahead);
+    kern<<<(unsigned)g, 2 * NT, smem, h->stream>>>(h->wmap, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], 2.0 / (double)h->n, 1, (int)ntiles);
     return check_launch(h);
 }
 
@@ -696,6 +677,8 @@ int prepare_kernels(dnslab *h)
     }
     if ((rc = poisson_solve(h, h->d, h->p, h->p, true))) return rc;
     if ((rc = poisson_solve(h, h->d, h->p, h->p, false))) return rc; // dnslab_poisson: never the dense prologue
+    // without a tensor map for W (no driver entry point) the solve takes the five single-axis passes, which need none
+    if (h->f_ny1 > 0 && h->P.ny / h->f_ny1 > 1 && !h->wmap_ok) h->f_ny1 = 0;
     {
         // dnslab_rfft3 / dnslab_irfft3 always take the single-axis passes, along z too
         const int keep = h->f_ny1;

@@ -180,12 +180,19 @@ template <int L, int E, int NS> struct NextRadix {
 // Full transform of one line held as x[e] <-> element tid + e*T, exchanging through `sm`
 // (SM::at(n) gives a reference to the shared slot of logical element n of this thread's line).
 // All threads that share the view must call this together (sm.sync() is a barrier among them).
-template <int L, int E, int DIR, int NS, class SM> __device__ __forceinline__ void fft_line(c2 (&x)[E], int tid, const c2 *__restrict__ tw, SM &sm)
+// `before_exchange` runs once, after the first radix stage and before anything is written to the exchange area (a caller
+// whose exchange area is still being read by someone else waits there).
+struct NoHook {
+    __device__ __forceinline__ void operator()() const {}
+};
+template <int L, int E, int DIR, int NS, class SM, class HOOK = NoHook>
+__device__ __forceinline__ void fft_line(c2 (&x)[E], int tid, const c2 *__restrict__ tw, SM &sm, HOOK before_exchange = HOOK())
 {
     constexpr int T = L / E;
     constexpr int R = NextRadix<L, E, NS>::value;
     constexpr int Q = E / R;
     stage<L, E, R, NS, DIR, SM::TWPOW, tw_in_smem<SM>::value>(x, tid, tw);
+    before_exchange();
     if constexpr (NS * R < L) {
 #pragma unroll
         for (int q = 0; q < Q; ++q) {
@@ -282,10 +289,6 @@ __device__ __forceinline__ void prefetch_l2(const void *p, unsigned bytes)
 {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(p), "r"(bytes) : "memory");
 }
-// The same for one cache line, as an ordinary per-lane instruction (the bulk form runs on the uniform datapath: a
-// warp whose lanes hold different addresses executes it once per lane, 25 instructions per element in k_fft_yz_solve)
-__device__ __forceinline__ void prefetch_l2_line(const void *p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p) : "memory"); }
-
 // x pass: lines of L = nx/2 complex numbers, contiguous.  NL lines per block, one line per T consecutive
 // threads, so the exchanges of a line never leave its warp (or its named barrier).
 //   FWD with PROLOGUE: in = d (real array viewed as complex), r = eq9_rhs(...) computed on load.
@@ -511,9 +514,18 @@ __global__ void __launch_bounds__(LX *NY1 / 16, (LX * NY1 / 16 <= 256 ? 2 : 1)) 
     }
 }
 
-// k_fft_yz_solve: one block per (ky1, tile of XT adjacent kx): the NY0 LZ XT values (kx, y0, z) of the rows
-// ky1 NY0 + y0 -- forward transform over y0 (in registers: a thread first holds all NY0 values of 16/NY0 z planes),
-// forward over z, multiplication by inv_n / lambda, and both transforms backwards.  Shared-memory tile [z][ky0][kx].
+// k_fft_yz_solve: the middle pass.  A tile is the NY0 LZ XT values (kx, y0, z) of the rows ky1 NY0 + y0 for XT adjacent kx
+// (XT = 2 on 512x256x128: 4096 points, 64 KB); the complex array is a rank-3 tensor (2 mx doubles, ny, nz) and one TMA box
+// (2 XT, NY0, LZ) is the whole tile, landing dense as [z][y0][xl] and leaving the same way: no load or store instruction
+// touches global memory and no register waits on one, so 32-byte runs cost the LSU nothing.  A dense tile is
+// conflict-free for threads that hold a z line (lanes on adjacent (xl, y0)), so z is transformed FIRST, straight out of
+// the landing buffer; the tile is then exchanged through a padded layout [z][y0][xl] (+XT per z) to threads that hold all
+// NY0 values of 16/NY0 planes: y0 transform, multiplication by inv_n / lambda, and everything backwards.
+// The block is persistent and works as two groups of NT threads.  Each group transforms its own tile stream (tiles
+// n = 0, 1, 2, ... of the block alternate between the groups) in its own work buffer; one landing buffer is shared: as soon
+// as a group has taken its tile out of it into registers, the box of the OTHER group's next tile is requested, so a load
+// is always in flight while both groups compute, and the store of a finished tile drains while its group works on the
+// first radix stage of the next one.  Group-wide named barriers only; one mbarrier per group for its loads.
 template <int N, int DIR> __device__ __forceinline__ void dft_small(c2 *v)
 {
     if constexpr (N == 2) {
@@ -527,198 +539,134 @@ template <int N, int DIR> __device__ __forceinline__ void dft_small(c2 *v)
     }
 }
 
-template <int STRIDE> struct SmStride {
+// Plane stride of the padded layout, in complex numbers: NY0 XT plus XT when XT < 8, so that the quarter-warps of both
+// layouts hit 32 different banks -- unless the padded buffers would not fit the SM (long z, few rows: the pad is then
+// half of a plane), where the y0 phase lives with two-way conflicts instead.
+template <int NY0, int LZ, int XT> struct YzLayout {
+    static constexpr int DROW = NY0 * XT;
+    static constexpr int padded = DROW + (XT < 8 ? XT : 0);
+    static constexpr size_t bytes_with(int zrow) { return ((size_t)LZ * DROW + 2 * (size_t)((LZ * zrow + 7) / 8 * 8) + LZ) * sizeof(c2) + LZ * sizeof(double); }
+    static constexpr int ZROW = bytes_with(padded) <= 227 * 1024 ? padded : DROW;
+    static constexpr int WBUF = (LZ * ZROW + 7) / 8 * 8; // work buffer of a group, in complex numbers (a multiple of 128 bytes)
+    static constexpr size_t SMEM = bytes_with(ZROW);     // landing buffer, two work buffers, z twiddles, z eigenvalue parts
+};
+
+template <int STRIDE> struct SmStrideBar {
     static constexpr bool TWPOW = false, TWSMEM = true; // all lanes of a warp share a z butterfly: table look-ups broadcast
     c2 *base;
+    int bar, nthreads;
     __device__ __forceinline__ c2 &at(int n) { return base[n * STRIDE]; }
-    __device__ __forceinline__ void sync() { __syncthreads(); }
+    __device__ __forceinline__ void sync() { asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(nthreads) : "memory"); }
 };
 
 template <int NY0, int LZ, int XT>
-__global__ void __launch_bounds__(XT *NY0 *LZ / 16, (XT * NY0 * LZ / 16 <= 256 ? 2 : 1))
-    k_fft_yz_solve(c2 *__restrict__ data, const c2 *__restrict__ twz, int mx, int ny, const double *__restrict__ ex, const double *__restrict__ ey,
-                   const double *__restrict__ ez, double inv_n, int rev, int ahead)
-{
-    constexpr int E = 16, G = E / NY0, ZQ = LZ / G, T = LZ / E, NT = XT * NY0 * LZ / E;
-    // one z plane of the tile: NY0 XT numbers, padded so that the quarter-warps of both layouts hit 32 different banks
-    constexpr int ZROW = NY0 * XT + (XT < 8 ? XT : 0);
-    static_assert(NY0 >= 2 && NY0 <= 16 && LZ >= 32, "unsupported split");
-    extern __shared__ double2 smem[];
-    c2 *stw = smem + LZ * ZROW;                         // z twiddles exp(-2 pi i t/LZ)
-    double *sez = reinterpret_cast<double *>(stw + LZ); // z eigenvalue parts
-    const int ny1 = ny / NY0, xtiles = mx / XT;
-    const unsigned bid = rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
-    const int xt = bid % xtiles, ky1 = bid / xtiles;
-    const int t = threadIdx.x, xl = t % XT, rest = t / XT;
-    const int zq = rest;                          // first layout: all y0 of the planes zq + g ZQ
-    const int ky0 = rest % NY0, tid = rest / NY0; // second layout: planes tid + e T of one ky0
-    const size_t zstride = (size_t)mx * ny;
-    c2 *g1 = data + (size_t)ky1 * NY0 * mx + (size_t)xt * XT + xl;
-    c2 x[E];
-#pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int y0 = 0; y0 < NY0; ++y0) x[g * NY0 + y0] = g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx];
-    for (int q = t; q < LZ; q += NT) {
-        sez[q] = ez[q];
-        stw[q] = twz[q];
-    }
-    {
-        // While this tile is computed, ask L2 for the tile of the block `ahead` places behind in launch order (the one
-        // that takes over an SM about when this block retires): LZ NY0 runs of XT complex numbers, one request per
-        // 128 bytes of each run.
-        const unsigned nb = blockIdx.x + ahead;
-        if (ahead > 0 && nb < gridDim.x) {
-            const unsigned nbid = rev ? gridDim.x - 1 - nb : nb;
-            const c2 *nt = data + (size_t)(nbid / xtiles) * NY0 * mx + (size_t)(nbid % xtiles) * XT;
-            constexpr int PER_RUN = XT >= 8 ? XT / 8 : 1, RUNS = LZ * NY0, REQ = RUNS * PER_RUN;
-#pragma unroll
-            for (int q0 = 0; q0 < (REQ + NT - 1) / NT; ++q0) {
-                const int q = t + q0 * NT, run = q / PER_RUN, part = q % PER_RUN; // (z, y0) = (run / NY0, run % NY0)
-                if (q < REQ) prefetch_l2_line(nt + (size_t)(run / NY0) * zstride + (size_t)(run % NY0) * mx + part * 8);
-            }
-        }
-    }
-#pragma unroll
-    for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
-#pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int q = 0; q < NY0; ++q) smem[(zq + g * ZQ) * ZROW + q * XT + xl] = x[g * NY0 + q];
-    __syncthreads();
-    SmStride<ZROW> sm{smem + ky0 * XT + xl};
-#pragma unroll
-    for (int e = 0; e < E; ++e) x[e] = sm.at(tid + e * T);
-    __syncthreads();
-    fft_line<LZ, E, -1, 1, SmStride<ZROW>>(x, tid, stw, sm);
-    {
-        const int m = xt * XT + xl, ky = ky1 + ny1 * ky0;
-        const double exy = __ldg(&ex[m]) + __ldg(&ey[ky]);
-        const bool null_xy = (m == 0) && (((2 * ky) & (ny - 1)) == 0);
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            const int kz = tid + e * T;
-            const double lam = -(exy + sez[kz]);
-            const bool null = null_xy && (((2 * kz) & (LZ - 1)) == 0);
-            const double sc = inv_n * rcp_newton(lam);
-            x[e].x = null ? 0.0 : x[e].x * sc;
-            x[e].y = null ? 0.0 : x[e].y * sc;
-        }
-    }
-    fft_line<LZ, E, +1, 1, SmStride<ZROW>>(x, tid, stw, sm);
-#pragma unroll
-    for (int e = 0; e < E; ++e) sm.at(tid + e * T) = x[e];
-    __syncthreads();
-#pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = smem[(zq + g * ZQ) * ZROW + q * XT + xl];
-#pragma unroll
-    for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
-#pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int y0 = 0; y0 < NY0; ++y0) g1[(size_t)(zq + g * ZQ) * zstride + (size_t)y0 * mx] = x[g * NY0 + y0];
-}
-
-// k_fft_zy_solve_tma: the same middle pass with its tile moved by TMA.  The complex array is a rank-3 tensor
-// (2 mx doubles, ny, nz); one box (2 XT, NY0, LZ) is the whole tile, landing dense as [z][y0][xl].  A dense tile is
-// conflict-free for threads that hold a z line (lanes on adjacent (xl, y0)), so z is transformed FIRST here, straight out
-// of the landing buffer, and y0 second (through the padded layout of the kernel above); the result goes back the same way
-// and leaves by one TMA store.  No load or store instruction touches global memory, no register waits on one: runs of
-// XT = 2 numbers (32 bytes) cost the LSU nothing, so tiles of 4096 points -- two blocks per SM -- become affordable.
-template <int NY0, int LZ, int XT>
-__global__ void __launch_bounds__(XT *NY0 *LZ / 16, (XT * NY0 * LZ / 16 <= 256 ? 2 : 1))
-    k_fft_zy_solve_tma(const __grid_constant__ CUtensorMap map, const c2 *__restrict__ twz, int mx, int ny, const double *__restrict__ ex,
-                       const double *__restrict__ ey, const double *__restrict__ ez, double inv_n, int rev)
+__global__ void __launch_bounds__(2 * XT * NY0 * LZ / 16, 1)
+    k_fft_yz_solve(const __grid_constant__ CUtensorMap map, const c2 *__restrict__ twz, int mx, int ny, const double *__restrict__ ex,
+                       const double *__restrict__ ey, const double *__restrict__ ez, double inv_n, int rev, int ntiles)
 {
     using namespace dnstma;
     constexpr int E = 16, G = E / NY0, ZQ = LZ / G, T = LZ / E, NT = XT * NY0 * LZ / E;
-    constexpr int DROW = NY0 * XT;                     // one z plane of the dense (TMA) layout
-    constexpr int ZROW = NY0 * XT + (XT < 8 ? XT : 0); // and of the padded layout between the z and the y0 transform
-    constexpr int ZB = LZ > 256 ? 256 : LZ;            // planes per box (a box extent is at most 256)
+    constexpr int DROW = NY0 * XT, ZROW = YzLayout<NY0, LZ, XT>::ZROW, WBUF = YzLayout<NY0, LZ, XT>::WBUF, ZB = LZ > 256 ? 256 : LZ;
     static_assert(NY0 >= 2 && NY0 <= 16 && LZ >= 32, "unsupported split");
     extern __shared__ __align__(128) double2 smem[];
-    __shared__ __align__(8) uint64_t mbar;
-    c2 *stw = smem + LZ * ZROW;                         // z twiddles exp(-2 pi i t/LZ)
+    __shared__ __align__(8) uint64_t full[2];
+    c2 *land = smem;                                    // dense landing buffer [z][y0][xl]
+    c2 *stw = smem + LZ * DROW + 2 * WBUF;              // z twiddles
     double *sez = reinterpret_cast<double *>(stw + LZ); // z eigenvalue parts
-    double *sey = sez + LZ;                             // y eigenvalue parts of this block's NY0 frequencies ky1 + ny1 ky0
     const int ny1 = ny / NY0, xtiles = mx / XT;
-    const unsigned bid = rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
-    const int xt = bid % xtiles, ky1 = bid / xtiles;
-    const int t = threadIdx.x, xl = t % XT, rest = t / XT;
-    const int y0 = rest % NY0, tid = rest / NY0; // z layout: planes tid + e T of one (xl, y0)
-    const int zq = rest;                         // y0 layout: all NY0 values of the planes zq + g ZQ
-    if (t == 0) {
-        mbar_init(&mbar, 1);
-        mbar_fence_init();
-        mbar_arrive_expect_tx(&mbar, (unsigned)(LZ * DROW * sizeof(c2)));
+    const int grp = threadIdx.x / NT, t = threadIdx.x - grp * NT;
+    c2 *work = smem + LZ * DROW + grp * WBUF;
+    const int xl = t % XT, rest = t / XT;
+    const int y0 = rest % NY0, tid = rest / NY0, zq = rest;
+    auto tile_of = [&](int n) { // the block's n-th tile, or -1
+        const long q = (long)blockIdx.x + (long)n * gridDim.x;
+        return q < ntiles ? (int)(rev ? ntiles - 1 - q : q) : -1;
+    };
+    auto request = [&](int n) { // thread-level: ask for the box of the block's n-th tile (if any) into the landing buffer
+        const int tl = tile_of(n);
+        if (tl < 0) return;
+        uint64_t *bar = &full[n & 1];
+        mbar_arrive_expect_tx(bar, (unsigned)(LZ * DROW * sizeof(c2)));
 #pragma unroll
-        for (int z0 = 0; z0 < LZ; z0 += ZB) tma_load_3d(smem + z0 * DROW, &map, &mbar, 2 * xt * XT, ky1 * NY0, z0);
+        for (int z0 = 0; z0 < LZ; z0 += ZB) tma_load_3d(land + z0 * DROW, &map, bar, 2 * (tl % xtiles) * XT, (tl / xtiles) * NY0, z0);
+    };
+    if (threadIdx.x == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        mbar_fence_init();
+        request(0);
     }
-    for (int q = t; q < LZ; q += NT) {
+    for (int q = threadIdx.x; q < LZ; q += 2 * NT) {
         sez[q] = ez[q];
         stw[q] = twz[q];
     }
-    if (t < NY0) sey[t] = ey[ky1 + ny1 * t];
-    __syncthreads(); // tables, and the initialised barrier, are visible to every thread
-    mbar_wait(&mbar, 0);
-    SmStride<DROW> sd{smem + y0 * XT + xl};
-    c2 x[E];
-#pragma unroll
-    for (int e = 0; e < E; ++e) x[e] = sd.at(tid + e * T);
     __syncthreads();
-    fft_line<LZ, E, -1, 1, SmStride<DROW>>(x, tid, stw, sd);
+    SmStrideBar<DROW> sl{land + y0 * XT + xl, 1 + grp, NT};
+    SmStrideBar<DROW> sd{work + y0 * XT + xl, 1 + grp, NT};
+    for (int n = grp; tile_of(n) >= 0; n += 2) {
+        const int tl = tile_of(n), xt = tl % xtiles, ky1 = tl / xtiles;
+        mbar_wait(&full[grp], (n >> 1) & 1);
+        c2 x[E];
 #pragma unroll
-    for (int e = 0; e < E; ++e) smem[(tid + e * T) * ZROW + y0 * XT + xl] = x[e];
-    __syncthreads();
+        for (int e = 0; e < E; ++e) x[e] = sl.at(tid + e * T);
+        sd.sync(); // the landing buffer is consumed
+        if (t == 0) request(n + 1);
+        fft_line<LZ, E, -1, 1, SmStrideBar<DROW>>(x, tid, stw, sd, [&]() {
+            if (t == 0) tma_store_wait_read(); // the store of this group's previous tile has read the work buffer
+            sd.sync();
+        });
 #pragma unroll
-    for (int g = 0; g < G; ++g)
+        for (int e = 0; e < E; ++e) work[(tid + e * T) * ZROW + y0 * XT + xl] = x[e];
+        sd.sync();
 #pragma unroll
-        for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = smem[(zq + g * ZQ) * ZROW + q * XT + xl];
+        for (int g = 0; g < G; ++g)
 #pragma unroll
-    for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
-    {
-        const int m = xt * XT + xl;
-        const double exm = __ldg(&ex[m]);
+            for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = work[(zq + g * ZQ) * ZROW + q * XT + xl];
 #pragma unroll
-        for (int g = 0; g < G; ++g) {
-            const int kz = zq + g * ZQ;
-            const double exz = exm + sez[kz];
-            const bool null_xz = (m == 0) && (((2 * kz) & (LZ - 1)) == 0);
+        for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
+        {
+            const int m = xt * XT + xl;
+            const double exm = __ldg(&ex[m]);
 #pragma unroll
-            for (int q = 0; q < NY0; ++q) {
-                const int ky = ky1 + ny1 * q;
-                const double lam = -(exz + sey[q]);
-                const bool null = null_xz && (((2 * ky) & (ny - 1)) == 0);
-                const double sc = inv_n * rcp_newton(lam);
-                x[g * NY0 + q].x = null ? 0.0 : x[g * NY0 + q].x * sc;
-                x[g * NY0 + q].y = null ? 0.0 : x[g * NY0 + q].y * sc;
+            for (int g = 0; g < G; ++g) {
+                const int kz = zq + g * ZQ;
+                const double exz = exm + sez[kz];
+                const bool null_xz = (m == 0) && (((2 * kz) & (LZ - 1)) == 0);
+#pragma unroll
+                for (int q = 0; q < NY0; ++q) {
+                    const int ky = ky1 + ny1 * q;
+                    const double lam = -(exz + __ldg(&ey[ky]));
+                    const bool null = null_xz && (((2 * ky) & (ny - 1)) == 0);
+                    const double sc = inv_n * rcp_newton(lam);
+                    x[g * NY0 + q].x = null ? 0.0 : x[g * NY0 + q].x * sc;
+                    x[g * NY0 + q].y = null ? 0.0 : x[g * NY0 + q].y * sc;
+                }
             }
         }
+#pragma unroll
+        for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int q = 0; q < NY0; ++q) work[(zq + g * ZQ) * ZROW + q * XT + xl] = x[g * NY0 + q];
+        sd.sync();
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = work[(tid + e * T) * ZROW + y0 * XT + xl];
+        sd.sync();
+        fft_line<LZ, E, +1, 1, SmStrideBar<DROW>>(x, tid, stw, sd);
+#pragma unroll
+        for (int e = 0; e < E; ++e) sd.at(tid + e * T) = x[e];
+        fence_proxy_async();
+        sd.sync();
+        if (t == 0) {
+#pragma unroll
+            for (int z0 = 0; z0 < LZ; z0 += ZB) tma_store_3d(&map, work + z0 * DROW, 2 * xt * XT, ky1 * NY0, z0);
+            tma_store_commit();
+        }
     }
-#pragma unroll
-    for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
-#pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int q = 0; q < NY0; ++q) smem[(zq + g * ZQ) * ZROW + q * XT + xl] = x[g * NY0 + q];
-    __syncthreads();
-#pragma unroll
-    for (int e = 0; e < E; ++e) x[e] = smem[(tid + e * T) * ZROW + y0 * XT + xl];
-    __syncthreads();
-    fft_line<LZ, E, +1, 1, SmStride<DROW>>(x, tid, stw, sd);
-#pragma unroll
-    for (int e = 0; e < E; ++e) sd.at(tid + e * T) = x[e];
-    fence_proxy_async();
-    __syncthreads();
-    if (t == 0) {
-#pragma unroll
-        for (int z0 = 0; z0 < LZ; z0 += ZB) tma_store_3d(&map, smem + z0 * DROW, 2 * xt * XT, ky1 * NY0, z0);
-        tma_store_commit();
-        tma_store_wait_read();
-    }
+    if (t == 0) tma_store_wait_read();
 }
+
 
 // ---------------------------------------------------------------------------------------
 // Real-to-complex entry points (dnslab_rfft3 / dnslab_irfft3): the transform itself, apart from the solve.
