@@ -581,8 +581,9 @@ int launch_eq9_sparse(dnslab *h, const double *p, bool first)
     while ((1 << lgx) < h->P.nx) ++lgx;
     while ((1 << lgy) < h->P.ny) ++lgy;
     ProfScope ps(h, DNSLAB_K_EQ9);
-    const int per = 256 * dnsst::EQ9_ITEMS;
-    const unsigned grid = (unsigned)((h->nb + per - 1) / per);
+    // one wave: 8 blocks of 256 threads per SM, never more blocks than the list needs
+    unsigned grid = (unsigned)((h->nb + 255) / 256);
+    if (grid > 8u * (unsigned)h->nsm) grid = 8u * (unsigned)h->nsm;
     const double r2x = 1.0 / (2.0 * h->P.dx), r2y = 1.0 / (2.0 * h->P.dy), r2z = 1.0 / (2.0 * h->P.dz);
     if (first) dnsst::k_eq9_sparse<true><<<grid, 256, 0, h->stream>>>(h->d, p, h->blist, h->bsave, h->nb, h->P.nx, h->P.ny, h->P.nz, lgx, lgy, r2x, r2y, r2z);
     else dnsst::k_eq9_sparse<false><<<grid, 256, 0, h->stream>>>(h->d, p, h->blist, h->bsave, h->nb, h->P.nx, h->P.ny, h->P.nz, lgx, lgy, r2x, r2y, r2z);
@@ -759,12 +760,13 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
         while (bx * by * bz < 256 && by < (unsigned)params->ny && by <= bz) by *= 2;
         while (bx * by * bz < 256 && bz < (unsigned)params->nz) bz *= 2;
         h->rk_block = dim3(bx, by, bz);
-        // marching kernel for nx >= 64: enough blocks for >= 6 waves of 2 blocks per SM, at least 8 planes each
-        // (16 planes per block is the best of 8...128 on 512x256x128)
+        // marching kernel for nx >= 64: 16 planes per block (the best of 8...128 on 512x256x128, and on 1024x512x256, where
+        // 128 planes per block -- 2048 blocks either way -- measured 2.41 instead of 2.15 ms per stage), 8 when that leaves
+        // fewer than 6 waves of 2 blocks per SM
         h->rk_kc = 0;
         if (params->nx >= dnsst::RKM_TX) {
             const long tiles = (long)(params->nx / dnsst::RKM_TX) * (params->ny / dnsst::RKM_TY);
-            int kc = params->nz;
+            int kc = params->nz < 16 ? params->nz : 16;
             while (kc > 8 && tiles * (params->nz / kc) < 6L * 2 * prop.multiProcessorCount) kc /= 2;
             h->rk_kc = kc;
         }

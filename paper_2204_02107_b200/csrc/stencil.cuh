@@ -527,56 +527,44 @@ __global__ void __launch_bounds__(256) k_div(const double *__restrict__ u, const
 // The first iteration of a step saves d at those cells (`save`), later ones restore it from there, and
 // r overwrites d in place: everywhere else r == d already, so the forward x pass reads one plain array.
 // face: bit0 beta(cell), bit1/2 beta(x+1/x-1), bit3/4 beta(y+1/y-1), bit5/6 beta(z+1/z-1).
-constexpr int EQ9_ITEMS = 1; // records per thread (4 with all loads issued together needs ~100 registers and measured slower: occupancy matters more here)
+// The kernel is a chain of two memory latencies (record, then d / p and its neighbours) and nothing else, so the grid is
+// one wave of blocks that stride through the list and each thread asks for its NEXT record before it works on the current
+// one: the two latencies overlap (measured on 512x256x128, 1.5 M records: see DESIGN.md section 6).
 template <bool FIRST>
 __global__ void __launch_bounds__(256) k_eq9_sparse(double *__restrict__ d, const double *__restrict__ p, const unsigned long long *__restrict__ rec,
                                                     double *__restrict__ save, int nlist, int nx, int ny, int nz, int lgx, int lgy,
                                                     double r2x, double r2y, double r2z)
 {
-    const int base = blockIdx.x * (256 * EQ9_ITEMS) + threadIdx.x;
-    unsigned long long rc[EQ9_ITEMS];
-#pragma unroll
-    for (int it = 0; it < EQ9_ITEMS; ++it) {
-        const int n = base + it * 256;
-        rc[it] = n < nlist ? __ldg(&rec[n]) : 0x7full << 32;
-    }
-    double dv[EQ9_ITEMS], pc[EQ9_ITEMS], pn[EQ9_ITEMS][6];
-#pragma unroll
-    for (int it = 0; it < EQ9_ITEMS; ++it) {
-        const int n = base + it * 256;
-        const uint32_t oo = (uint32_t)rc[it];
-        const unsigned ff = (unsigned)(rc[it] >> 32);
-        const int i = oo & (nx - 1), j = (oo >> lgx) & (ny - 1), k = oo >> (lgx + lgy);
-        const size_t row = (size_t)nx * ((size_t)j + (size_t)ny * k);
-        dv[it] = pc[it] = 0.0;
-#pragma unroll
-        for (int q = 0; q < 6; ++q) pn[it][q] = 0.0;
-        if (n < nlist) {
-            dv[it] = FIRST ? d[oo] : save[n];
-            pc[it] = __ldg(&p[oo]);
-            if (!(ff & 2)) pn[it][0] = __ldg(&p[row + ((i + 2) & (nx - 1))]);
-            if (!(ff & 4)) pn[it][1] = __ldg(&p[row + ((i - 2) & (nx - 1))]);
-            if (!(ff & 8)) pn[it][2] = __ldg(&p[(size_t)nx * ((size_t)((j + 2) & (ny - 1)) + (size_t)ny * k) + i]);
-            if (!(ff & 16)) pn[it][3] = __ldg(&p[(size_t)nx * ((size_t)((j - 2) & (ny - 1)) + (size_t)ny * k) + i]);
-            if (!(ff & 32)) pn[it][4] = __ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k + 2) & (nz - 1))) + i]);
-            if (!(ff & 64)) pn[it][5] = __ldg(&p[(size_t)nx * ((size_t)j + (size_t)ny * ((k - 2) & (nz - 1))) + i]);
-        }
-    }
-#pragma unroll
-    for (int it = 0; it < EQ9_ITEMS; ++it) {
-        const int n = base + it * 256;
-        if (n >= nlist) continue;
-        const uint32_t oo = (uint32_t)rc[it];
-        const unsigned ff = (unsigned)(rc[it] >> 32);
-        if (FIRST) save[n] = dv[it];
+    // neighbour offsets two cells away, periodic: extents are powers of two and the whole array has fewer than 2^32
+    // elements, so each axis is a bit field of the linear index and the wrap is a masked add
+    const uint32_t mx_ = (uint32_t)nx - 1u, my_ = ((uint32_t)ny - 1u) << lgx, mz_ = ((uint32_t)nz - 1u) << (lgx + lgy);
+    const uint32_t sx = 2u, sy = 2u << lgx, sz = 2u << (lgx + lgy);
+    const int stride = gridDim.x * 256;
+    int n = blockIdx.x * 256 + threadIdx.x;
+    unsigned long long rc = n < nlist ? __ldg(&rec[n]) : 0ull;
+    for (; n < nlist; n += stride) {
+        const unsigned long long cur = rc;
+        if (n + stride < nlist) rc = __ldg(&rec[n + stride]);
+        const uint32_t oo = (uint32_t)cur;
+        const unsigned ff = (unsigned)(cur >> 32);
+        const double dv = FIRST ? d[oo] : save[n];
+        const double pc = __ldg(&p[oo]);
+        double pn[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        if (!(ff & 2)) pn[0] = __ldg(&p[(oo & ~mx_) | ((oo + sx) & mx_)]);
+        if (!(ff & 4)) pn[1] = __ldg(&p[(oo & ~mx_) | ((oo - sx) & mx_)]);
+        if (!(ff & 8)) pn[2] = __ldg(&p[(oo & ~my_) | ((oo + sy) & my_)]);
+        if (!(ff & 16)) pn[3] = __ldg(&p[(oo & ~my_) | ((oo - sy) & my_)]);
+        if (!(ff & 32)) pn[4] = __ldg(&p[(oo & ~mz_) | ((oo + sz) & mz_)]);
+        if (!(ff & 64)) pn[5] = __ldg(&p[(oo & ~mz_) | ((oo - sz) & mz_)]);
+        if (FIRST) save[n] = dv;
         double gxp = 0.0, gxm = 0.0, gyp = 0.0, gym = 0.0, gzp = 0.0, gzm = 0.0;
-        if (!(ff & 2)) gxp = (pn[it][0] - pc[it]) * r2x;
-        if (!(ff & 4)) gxm = (pc[it] - pn[it][1]) * r2x;
-        if (!(ff & 8)) gyp = (pn[it][2] - pc[it]) * r2y;
-        if (!(ff & 16)) gym = (pc[it] - pn[it][3]) * r2y;
-        if (!(ff & 32)) gzp = (pn[it][4] - pc[it]) * r2z;
-        if (!(ff & 64)) gzm = (pc[it] - pn[it][5]) * r2z;
-        d[oo] = dv[it] + ((gxp - gxm) * r2x + (gyp - gym) * r2y + (gzp - gzm) * r2z);
+        if (!(ff & 2)) gxp = (pn[0] - pc) * r2x;
+        if (!(ff & 4)) gxm = (pc - pn[1]) * r2x;
+        if (!(ff & 8)) gyp = (pn[2] - pc) * r2y;
+        if (!(ff & 16)) gym = (pc - pn[3]) * r2y;
+        if (!(ff & 32)) gzp = (pn[4] - pc) * r2z;
+        if (!(ff & 64)) gzm = (pc - pn[5]) * r2z;
+        d[oo] = dv + ((gxp - gxm) * r2x + (gyp - gym) * r2y + (gzp - gzm) * r2z);
     }
 }
 
