@@ -105,8 +105,8 @@ def ncu_traffic(path, cls, case):
         return None, f"no {cls} kernel in {os.path.relpath(path, ROOT)}"
     # a capture of another grid is not this workload's traffic: the RK kernels' grids give the cell count away
     meta = os.path.splitext(path)[0] + ".md"
-    if os.path.exists(meta) and case["name"] not in open(meta).read():
-        return None, f"{os.path.relpath(meta, ROOT)} does not name workload {case['name']}"
+    if not os.path.exists(meta) or case["name"] not in open(meta).read():
+        return None, f"{os.path.relpath(meta, ROOT)} does not name workload {case['name']}: the capture belongs to another workload"
     return sum(vals) / len(vals), f"{os.path.relpath(path, ROOT)}: mean of {len(vals)} launches"
 
 
@@ -510,7 +510,7 @@ def main():
     ap.add_argument("--mode", default="step", choices=["step", "reductions", "particles"],
                     help="step: the headline line; reductions / particles: the NEXT-3 / NEXT-4 lines")
     ap.add_argument("--particles", type=int, default=1000000, help="--mode particles: how many")
-    ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r02c_ncu_full_raw.csv"),
+    ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r02e_ncu_full_raw.csv"),
                     help="ncu --page raw --csv export of a --set full capture of this workload (roofline.traffic)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
