@@ -130,6 +130,8 @@ struct dnslab {
     void *tma_encode; // cuTensorMapEncodeTiled, fetched through cudaGetDriverEntryPoint at create (null: no TMA anywhere)
     bool wmap_ok;     // the tensor map of the transform array W is built (the middle pass of the two-pass solve moves its tiles by TMA)
     CUtensorMap wmap;
+    bool wmapz_ok;    // the same for the fused z pass without a split of y (box 2 XT x 1 x nz)
+    CUtensorMap wmapz;
     long long np;      // NEXT-4: attached particles (0: none); state is the caller's device array
     double *pstate, prho_f, pgrav[3];
     // optional per-launch timing (dnslab_profile): events bracketing every kernel, by class
@@ -287,6 +289,9 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
 }
 
 // ---- FFT passes -------------------------------------------------------------------------
+#ifndef DNSLAB_Z_TMA
+#define DNSLAB_Z_TMA 1
+#endif
 template <int L> constexpr int col_xt() { return L >= 1024 ? 4 : (L >= 256 ? 8 : 16); }
 
 // grid of a persistent pass: every SM filled with as many blocks as fit, never more blocks than tiles
@@ -391,8 +396,43 @@ template <int L, int XT> int launch_fft_z_solve_LX(dnslab *h, c2 *data)
     return check_launch(h);
 }
 
+// The fused z pass by TMA: k_fft_yz_solve without a split of y (NY0 = 1) -- persistent two-group blocks, tiles of 4096 points
+// (XT = 4096 / nz adjacent kx, at most 16) in and out as boxes of W's second tensor map.
+template <int L> int launch_fft_z_solve_tma(dnslab *h, c2 *data, bool *done)
+{
+    constexpr int XT = 4096 / L > 16 ? 16 : 4096 / L, NT = XT * L / 16, ZB = L > 256 ? 256 : L;
+    const int mx = h->P.nx / 2;
+    *done = false;
+    if (mx < XT || data != reinterpret_cast<c2 *>(h->W)) return DNSLAB_OK;
+    const size_t smem = dnsfft::YzLayout<1, L, XT>::SMEM;
+    auto kern = dnsfft::k_fft_yz_solve<1, L, XT>;
+    if (h->prepare) {
+        const cuuint64_t gdim[3] = {(cuuint64_t)(2 * mx), (cuuint64_t)h->P.ny, (cuuint64_t)h->P.nz};
+        const cuuint32_t box[3] = {(cuuint32_t)(2 * XT), 1u, (cuuint32_t)ZB};
+        h->wmapz_ok = encode_map3(h, &h->wmapz, (void *)data, gdim, box);
+        if (h->wmapz_ok) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        *done = h->wmapz_ok;
+        return DNSLAB_OK;
+    }
+    if (!h->wmapz_ok) return DNSLAB_OK;
+    *done = true;
+    const size_t ntiles = (size_t)(mx / XT) * h->P.ny;
+    size_t g = (size_t)h->nsm < ntiles ? (size_t)h->nsm : ntiles;
+    const size_t per_block = (ntiles + g - 1) / g;
+    g = (ntiles + per_block - 1) / per_block;
+    ProfScope ps(h, DNSLAB_K_FFT_Z);
+    kern<<<(unsigned)g, 2 * NT, smem, h->stream>>>(h->wmapz, h->tw[2], mx, h->P.ny, h->eig[0], h->eig[1], h->eig[2], 2.0 / (double)h->n,
+                                                  (FFT_REV >> 2) & 1, (int)ntiles);
+    return check_launch(h);
+}
+
 template <int L> int launch_fft_z_solve_L(dnslab *h, c2 *data)
 {
+    if constexpr (L >= 32 && DNSLAB_Z_TMA) {
+        bool done = false;
+        const int rc = launch_fft_z_solve_tma<L>(h, data, &done);
+        if (rc || (done && !h->prepare)) return rc;
+    }
     constexpr int XT = col_xt<L>();
     if (h->P.nx / 2 >= XT) return launch_fft_z_solve_LX<L, XT>(h, data);
     return launch_fft_z_solve_LX<L, 4>(h, data);
@@ -777,6 +817,7 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
     // kernel of small grids) every block copies its tiles with cp.async.
     h->tma_ok = false;
     h->wmap_ok = false;
+    h->wmapz_ok = false;
     h->tma_encode = nullptr;
     {
         void *fp = nullptr;

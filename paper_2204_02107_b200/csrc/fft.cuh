@@ -544,7 +544,7 @@ template <int N, int DIR> __device__ __forceinline__ void dft_small(c2 *v)
 // half of a plane), where the y0 phase lives with two-way conflicts instead.
 template <int NY0, int LZ, int XT> struct YzLayout {
     static constexpr int DROW = NY0 * XT;
-    static constexpr int padded = DROW + (XT < 8 ? XT : 0);
+    static constexpr int padded = DROW + (NY0 > 1 && XT < 8 ? XT : 0); // NY0 == 1: the padded layout is not used
     static constexpr size_t bytes_with(int zrow) { return ((size_t)LZ * DROW + 2 * (size_t)((LZ * zrow + 7) / 8 * 8) + LZ) * sizeof(c2) + LZ * sizeof(double); }
     static constexpr int ZROW = bytes_with(padded) <= 227 * 1024 ? padded : DROW;
     static constexpr int WBUF = (LZ * ZROW + 7) / 8 * 8; // work buffer of a group, in complex numbers (a multiple of 128 bytes)
@@ -567,7 +567,7 @@ __global__ void __launch_bounds__(2 * XT * NY0 * LZ / 16, 1)
     using namespace dnstma;
     constexpr int E = 16, G = E / NY0, ZQ = LZ / G, T = LZ / E, NT = XT * NY0 * LZ / E;
     constexpr int DROW = NY0 * XT, ZROW = YzLayout<NY0, LZ, XT>::ZROW, WBUF = YzLayout<NY0, LZ, XT>::WBUF, ZB = LZ > 256 ? 256 : LZ;
-    static_assert(NY0 >= 2 && NY0 <= 16 && LZ >= 32, "unsupported split");
+    static_assert(NY0 >= 1 && NY0 <= 16 && LZ >= 32, "unsupported split");
     extern __shared__ __align__(128) double2 smem[];
     __shared__ __align__(8) uint64_t full[2];
     c2 *land = smem;                                    // dense landing buffer [z][y0][xl]
@@ -615,44 +615,60 @@ __global__ void __launch_bounds__(2 * XT * NY0 * LZ / 16, 1)
             if (t == 0) tma_store_wait_read(); // the store of this group's previous tile has read the work buffer
             sd.sync();
         });
+        if constexpr (NY0 > 1) {
 #pragma unroll
-        for (int e = 0; e < E; ++e) work[(tid + e * T) * ZROW + y0 * XT + xl] = x[e];
-        sd.sync();
+            for (int e = 0; e < E; ++e) work[(tid + e * T) * ZROW + y0 * XT + xl] = x[e];
+            sd.sync();
 #pragma unroll
-        for (int g = 0; g < G; ++g)
+            for (int g = 0; g < G; ++g)
 #pragma unroll
-            for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = work[(zq + g * ZQ) * ZROW + q * XT + xl];
+                for (int q = 0; q < NY0; ++q) x[g * NY0 + q] = work[(zq + g * ZQ) * ZROW + q * XT + xl];
 #pragma unroll
-        for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
-        {
-            const int m = xt * XT + xl;
-            const double exm = __ldg(&ex[m]);
+            for (int g = 0; g < G; ++g) dft_small<NY0, -1>(x + g * NY0);
+            {
+                const int m = xt * XT + xl;
+                const double exm = __ldg(&ex[m]);
 #pragma unroll
-            for (int g = 0; g < G; ++g) {
-                const int kz = zq + g * ZQ;
-                const double exz = exm + sez[kz];
-                const bool null_xz = (m == 0) && (((2 * kz) & (LZ - 1)) == 0);
+                for (int g = 0; g < G; ++g) {
+                    const int kz = zq + g * ZQ;
+                    const double exz = exm + sez[kz];
+                    const bool null_xz = (m == 0) && (((2 * kz) & (LZ - 1)) == 0);
 #pragma unroll
-                for (int q = 0; q < NY0; ++q) {
-                    const int ky = ky1 + ny1 * q;
-                    const double lam = -(exz + __ldg(&ey[ky]));
-                    const bool null = null_xz && (((2 * ky) & (ny - 1)) == 0);
-                    const double sc = inv_n * rcp_newton(lam);
-                    x[g * NY0 + q].x = null ? 0.0 : x[g * NY0 + q].x * sc;
-                    x[g * NY0 + q].y = null ? 0.0 : x[g * NY0 + q].y * sc;
+                    for (int q = 0; q < NY0; ++q) {
+                        const int ky = ky1 + ny1 * q;
+                        const double lam = -(exz + __ldg(&ey[ky]));
+                        const bool null = null_xz && (((2 * ky) & (ny - 1)) == 0);
+                        const double sc = inv_n * rcp_newton(lam);
+                        x[g * NY0 + q].x = null ? 0.0 : x[g * NY0 + q].x * sc;
+                        x[g * NY0 + q].y = null ? 0.0 : x[g * NY0 + q].y * sc;
+                    }
                 }
             }
+#pragma unroll
+            for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
+#pragma unroll
+            for (int g = 0; g < G; ++g)
+#pragma unroll
+                for (int q = 0; q < NY0; ++q) work[(zq + g * ZQ) * ZROW + q * XT + xl] = x[g * NY0 + q];
+            sd.sync();
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = work[(tid + e * T) * ZROW + y0 * XT + xl];
+            sd.sync();
+        } else {
+            // no split of y (ny0 == 1, and the z pass of the five single-axis passes): the spectrum is complete in the z layout
+            const int m = xt * XT + xl;
+            const double exy = __ldg(&ex[m]) + __ldg(&ey[ky1]);
+            const bool null_xy = (m == 0) && (((2 * ky1) & (ny - 1)) == 0);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int kz = tid + e * T;
+                const double lam = -(exy + sez[kz]);
+                const bool null = null_xy && (((2 * kz) & (LZ - 1)) == 0);
+                const double sc = inv_n * rcp_newton(lam);
+                x[e].x = null ? 0.0 : x[e].x * sc;
+                x[e].y = null ? 0.0 : x[e].y * sc;
+            }
         }
-#pragma unroll
-        for (int g = 0; g < G; ++g) dft_small<NY0, +1>(x + g * NY0);
-#pragma unroll
-        for (int g = 0; g < G; ++g)
-#pragma unroll
-            for (int q = 0; q < NY0; ++q) work[(zq + g * ZQ) * ZROW + q * XT + xl] = x[g * NY0 + q];
-        sd.sync();
-#pragma unroll
-        for (int e = 0; e < E; ++e) x[e] = work[(tid + e * T) * ZROW + y0 * XT + xl];
-        sd.sync();
         fft_line<LZ, E, +1, 1, SmStrideBar<DROW>>(x, tid, stw, sd);
 #pragma unroll
         for (int e = 0; e < E; ++e) sd.at(tid + e * T) = x[e];
