@@ -91,6 +91,29 @@ def test_poisson_two_pass_shapes_match_oracle(shape):
     assert torch.equal(buf, p)
 
 
+@pytest.mark.parametrize("shape", [(128, 256, 512), (256, 64, 128), (512, 16, 64)])
+def test_poisson_persistent_passes_are_repeatable(shape):
+    """The middle pass (k_fft_yz_solve) is a persistent kernel whose two thread groups share a landing buffer and hand
+    tiles to each other through mbarriers and named barriers, with loads and stores in flight under the arithmetic.  A
+    missing wait would show as a result that depends on timing: 25 solves of the same right-hand side -- config 4's grid
+    (two-pass, NY0 = 16), a five-pass shape whose z pass takes the NY0 = 1 route, and one with several boxes per tile
+    (nz = 512) -- must agree bit for bit, in place and out of place."""
+    import torch
+    rng = np.random.default_rng(sum(shape) + 3)
+    rhs = torch.from_numpy(rng.standard_normal(shape)).cuda()
+    s = binding.Solver(shape, (0.11, 0.07, 0.05), 0.1, 0.1, 0.1)
+    first = s.poisson(rhs).clone()
+    for it in range(25):
+        if it % 2:
+            buf = rhs.clone()
+            s.poisson(buf, out=buf)
+        else:
+            buf = s.poisson(rhs)
+        s.synchronize()
+        assert torch.equal(buf, first), it
+    s.close()
+
+
 @pytest.mark.parametrize("shape", [(8, 8, 8), (16, 32, 64), (32, 8, 16), (8, 64, 128), (64, 16, 256), (32, 128, 512)])
 def test_rfft3_real_to_complex_transform_matches_oracle(shape):
     """dnslab_rfft3 / dnslab_irfft3: the real-to-complex transform on its own (north_star names one) against the oracle's
