@@ -289,9 +289,6 @@ template <int STAGE, bool ELIM> int launch_rk(dnslab *h, double *const *qs, doub
 }
 
 // ---- FFT passes -------------------------------------------------------------------------
-#ifndef DNSLAB_Z_TMA
-#define DNSLAB_Z_TMA 1
-#endif
 template <int L> constexpr int col_xt() { return L >= 1024 ? 4 : (L >= 256 ? 8 : 16); }
 
 // grid of a persistent pass: every SM filled with as many blocks as fit, never more blocks than tiles
@@ -428,7 +425,7 @@ template <int L> int launch_fft_z_solve_tma(dnslab *h, c2 *data, bool *done)
 
 template <int L> int launch_fft_z_solve_L(dnslab *h, c2 *data)
 {
-    if constexpr (L >= 32 && DNSLAB_Z_TMA) {
+    if constexpr (L >= 32) {
         bool done = false;
         const int rc = launch_fft_z_solve_tma<L>(h, data, &done);
         if (rc || (done && !h->prepare)) return rc;
@@ -649,10 +646,11 @@ int launch_filter(dnslab *h, double *const *in, double *const *out)
     }
     ProfScope ps(h, DNSLAB_K_FILTER);
     if (h->P.nx >= dnsst::FM_TX && h->P.ny >= dnsst::FM_TY) {
-        // z-marching kernel: 64 x 8 columns of one field; >= 4 waves of 4 blocks per SM, at least 8 planes per block
+        // z-marching kernel: 64 x 8 columns of one field; >= 3 waves of 4 blocks per SM, at least 8 planes per block
+        // (512x256x128: 64 planes per block 286 us, 32: 296 us, 16: 302 us, 8: 326 us, 128 -- 1.7 waves: 306 us)
         const long tiles = 4L * (h->P.nx / dnsst::FM_TX) * (h->P.ny / dnsst::FM_TY);
         int kc = h->P.nz;
-        while (kc > 8 && tiles * (h->P.nz / kc) < 16L * h->nsm) kc /= 2;
+        while (kc > 8 && tiles * (h->P.nz / kc) < 12L * h->nsm) kc /= 2;
         a.kc = kc;
         const dim3 blk(32, dnsst::FM_TY, 1);
         const dim3 grd(h->P.nx / dnsst::FM_TX, h->P.ny / dnsst::FM_TY, 4 * (h->P.nz / kc));
