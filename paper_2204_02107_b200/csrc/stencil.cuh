@@ -650,15 +650,15 @@ template <bool MASKED> __global__ void __launch_bounds__(256) k_filter_march(con
     const unsigned s0 = (unsigned)nx * ((y0 - 3 + r0) & (ny - 1)) + ((x0 - 4 + 2 * q0) & (nx - 1));
     const unsigned s1 = (unsigned)nx * ((y0 - 3 + r1) & (ny - 1)) + ((x0 - 4 + 2 * q1) & (nx - 1));
     const int d0 = r0 * FM_W + 2 * q0, d1 = r1 * FM_W + 2 * q1;
-    auto issue = [&](int n) { // plane k0+n into tile n % 6
+    auto issue = [&](int n, int buf) { // plane k0+n into tile `buf` (= n % 6)
         const double *src = f + plane * (size_t)((k0 + n) & (nz - 1));
-        double *dst = sm + (n % FM_NBUF) * FM_TILE;
+        double *dst = sm + buf * FM_TILE;
         cp_async16(dst + d0, src + s0);
         if (has1) cp_async16(dst + d1, src + s1);
     };
 #pragma unroll
     for (int n = 0; n < 5; ++n) {
-        issue(n);
+        issue(n, n);
         cp_async_commit();
     }
     double2 z[7]; // z[3] is the centre plane
@@ -669,22 +669,26 @@ template <bool MASKED> __global__ void __launch_bounds__(256) k_filter_march(con
 #pragma unroll
     for (int d = 0; d < 3; ++d) z[d + 4] = *reinterpret_cast<const double2 *>(sm + d * FM_TILE + own);
 
-    for (int t = 0; t < kc; ++t) {
-        const size_t pk = plane * (size_t)(k0 + t);
-        unsigned fA = 1, fB = 1;
-        if (MASKED) {
-            const uchar2 fv = *reinterpret_cast<const uchar2 *>(a.face + pk + col);
-            fA = fv.x;
-            fB = fv.y;
-        }
+    // tile indices t % 6, (t + 3) % 6, (t + 5) % 6 as running counters (a modulo by 6 per use cost ~15 instructions each);
+    // the face bytes of plane t + 1 are fetched while plane t is computed
+    int bc = 0, b3 = 3, b5 = 5;
+    size_t pk = plane * (size_t)k0 + col;
+    unsigned fnext = 0x0101;
+    if (MASKED) fnext = *reinterpret_cast<const unsigned short *>(a.face + pk);
+    for (int t = 0; t < kc; ++t, pk += plane) {
+        const unsigned fcur = fnext;
+        if (MASKED && t + 1 < kc) fnext = *reinterpret_cast<const unsigned short *>(a.face + pk + plane);
         cp_async_wait_one();
         __syncthreads(); // tile t+3 visible; every thread is done with tile t-1
-        if (t + 5 <= kc + 2) issue(t + 5);
+        if (t + 5 <= kc + 2) issue(t + 5, b5);
         cp_async_commit();
 #pragma unroll
         for (int d = 0; d < 6; ++d) z[d] = z[d + 1];
-        z[6] = *reinterpret_cast<const double2 *>(sm + ((t + 3) % FM_NBUF) * FM_TILE + own);
-        const double *sc = sm + (t % FM_NBUF) * FM_TILE + own;
+        z[6] = *reinterpret_cast<const double2 *>(sm + b3 * FM_TILE + own);
+        const double *sc = sm + bc * FM_TILE + own;
+        bc = bc == FM_NBUF - 1 ? 0 : bc + 1;
+        b3 = b3 == FM_NBUF - 1 ? 0 : b3 + 1;
+        b5 = b5 == FM_NBUF - 1 ? 0 : b5 + 1;
         const double2 xa = *reinterpret_cast<const double2 *>(sc - 4), xb = *reinterpret_cast<const double2 *>(sc - 2);
         const double2 xc = *reinterpret_cast<const double2 *>(sc + 2), xd = *reinterpret_cast<const double2 *>(sc + 4);
         const double2 c = z[3];
@@ -699,9 +703,9 @@ template <bool MASKED> __global__ void __launch_bounds__(256) k_filter_march(con
         const double szA = z[0].x - 6.0 * z[1].x + 15.0 * z[2].x - 20.0 * c.x + 15.0 * z[4].x - 6.0 * z[5].x + z[6].x;
         const double szB = z[0].y - 6.0 * z[1].y + 15.0 * z[2].y - 20.0 * c.y + 15.0 * z[4].y - 6.0 * z[5].y + z[6].y;
         double2 r;
-        r.x = (!MASKED || (fA & 1)) ? c.x + a.g * ((sxA + syA) + szA) : 0.0;
-        r.y = (!MASKED || (fB & 1)) ? c.y + a.g * ((sxB + syB) + szB) : 0.0;
-        *reinterpret_cast<double2 *>(o + pk + col) = r;
+        r.x = (!MASKED || (fcur & 1)) ? c.x + a.g * ((sxA + syA) + szA) : 0.0;
+        r.y = (!MASKED || (fcur & 0x100)) ? c.y + a.g * ((sxB + syB) + szB) : 0.0;
+        *reinterpret_cast<double2 *>(o + pk) = r;
     }
 }
 
