@@ -96,7 +96,7 @@ int dnslab_set_fields(dnslab_t *h, const double *u, const double *v, const doubl
 int dnslab_step(dnslab_t *h, int32_t n);
 
 /* One Poisson solve with the beta term off: p = F^-1[F[rhs]/lambda], null modes 0 (eq. 9 with
- * beta = 1).  rhs and p are DEVICE pointers to nx*ny*nz doubles; they may alias.  Does not
+ * beta = 1).  rhs and p are DEVICE pointers to nx*ny*nz doubles, 16-byte aligned; they may alias.  Does not
  * touch the solver's own pressure. */
 int dnslab_poisson(dnslab_t *h, const double *rhs, double *p);
 
