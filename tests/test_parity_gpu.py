@@ -235,6 +235,18 @@ def test_config5_full_size_one_step(record_property):
 
 
 # ------------------------------------------------------------------ variants and edge cases
+@pytest.mark.slow
+def test_twice_config5_268M_cells_one_step(record_property):
+    """Beyond the five configs: config 5's generator on 1024 x 1024 x 256 (268 M cells, 43 GB of workspace; ny at the
+    library's maximum of 1024, 32-bit element offsets up to 2^28), one step.  Needs about 90 GB of host memory for the
+    oracle and the comparison; skipped below 110 GB available."""
+    import psutil
+    avail = psutil.virtual_memory().available / 2 ** 30
+    if avail < 110:
+        pytest.skip(f"{avail:.0f} GB of host memory available, 110 GB wanted")
+    _full_size(cases.three_rooms(1024, 1024, 256), [1], record_property, "twice config 5, 1024x1024x256")
+
+
 def test_per_stage_projection_variant():
     case = cases.duct_room(32, 16, 16)
     for cp, got, ref in run_both(case, [1, 5], flags=2):
