@@ -1139,7 +1139,7 @@ int dnslab_courant(dnslab_t *h, double *co)
     {
         ProfScope ps(h, DNSLAB_K_REDUCE);
         size_t g = (h->n + 255) / 256;
-        if (g > (size_t)16 * h->nsm) g = (size_t)16 * h->nsm;
+        if (g > (size_t)4 * h->nsm) g = (size_t)4 * h->nsm; // few, long-running blocks: the shared threshold settles early
         dnsred::k_courant<<<(unsigned)g, 256, 0, h->stream>>>(h->Q[0], h->Q[1], h->Q[2], h->n, h->P.dx, h->P.dy, h->P.dz, res);
         if (int rc = check_launch(h)) return rc;
     }
