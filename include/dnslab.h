@@ -42,6 +42,7 @@ extern "C" {
 #define DNSLAB_ENOMEM (-2) /* workspace smaller than dnslab_workspace_bytes()                         */
 #define DNSLAB_ECUDA (-3)  /* a CUDA call or kernel launch failed (sticky error)                      */
 #define DNSLAB_EARCH (-4)  /* no device, or the current device is not compute capability 10.x         */
+#define DNSLAB_ELIMIT (-5) /* dnslab_scalar_stats_static: the box has more than DNSLAB_STATIC_MAX_ROWS rows     */
 
 #define DNSLAB_MAX_SOURCES 16
 
@@ -158,6 +159,45 @@ int dnslab_profile_read(dnslab_t *h, double *ms, int64_t *launches);
 int dnslab_courant(dnslab_t *h, double *co);
 int dnslab_set_dt(dnslab_t *h, double dt);
 int dnslab_scalar_stats(dnslab_t *h, const int32_t lo[3], const int32_t size[3], double out[3]);
+
+/* ---- The same statistic for callers that cannot give the library any device memory -----------------------------
+ * Everything else in this header runs out of a device workspace that the caller had to allocate for dnslab_create.
+ * Some callers have no way to do that, and must not trigger a cudaMalloc either:
+ *   - a monitor or co-processing plug-in that is handed borrowed field pointers (dnslab_fields) by a solver whose
+ *     owner has already given the whole HBM to its fields or to a framework's caching pool (config 5 of this repo
+ *     is such a "full-HBM working set"): a second workspace or a cudaMalloc simply fails with out-of-memory;
+ *   - code on a path where allocation is forbidden or too costly: cudaMalloc / cudaFree synchronise the whole
+ *     device and stall every stream of a running simulation, and they are illegal while a stream is being captured;
+ *   - hosts that account for every device byte up front (fixed memory budgets, MPS / MIG slices with a hard limit).
+ * dnslab_scalar_stats_static computes what dnslab_scalar_stats computes -- mean, population standard deviation and
+ * count of c over the fluid cells of an index box (reading R25) -- without a handle and
+ * without allocating: it calls no cudaMalloc, cudaFree or any routine that allocates.  Its scratch (one partial sum
+ * and one count per row of the box) is a fixed array inside the library's device image: 2 * DNSLAB_STATIC_MAX_ROWS
+ * doubles = 1 MiB, which every GPU that loads libdnslab.so holds until the process exits, whether this call is ever
+ * made or not.
+ *   c     DEVICE, nx*ny*nz doubles, x fastest (the layout at the top of this file); read only.
+ *   mask  DEVICE, nx*ny*nz bytes, non-zero = fluid; NULL = every cell is fluid; read only.
+ *   nx, ny, nz  powers of two within the limits given at dnslab_params_t; anything else: DNSLAB_EINVAL.
+ *   lo, size    HOST, the index box as in dnslab_scalar_stats (1 <= size[a] <= N_a, wraps modulo N).
+ *   cuda_stream a cudaStream_t (NULL = default stream); the call is ASYNCHRONOUS on it, no host synchronisation.
+ *   out   DEVICE, 3 doubles, caller-owned: mean, std, count (zeros for a box without fluid cells); also read by the
+ *         call itself between its passes, so nothing else may write it until the call has finished on the stream.
+ * Limit: size[1]*size[2] <= DNSLAB_STATIC_MAX_ROWS (65 536 rows: a full 256 x 256 cross-section, any length in x).
+ * A taller box returns DNSLAB_ELIMIT ("box has more rows ... than the static scratch array holds") and launches
+ * nothing; split it into slabs, or use dnslab_scalar_stats.
+ * First call on a device: the library looks up the device address of its array (cudaGetSymbolAddress) with that
+ * device current and remembers it; this one-time set-up is not a stream operation, so make the first call on each
+ * device before any stream capture begins.  The calling thread's current device must be the one c, mask and out
+ * live on.
+ * Sharing: all calls in the process use the same array on a device, and it keeps whatever the last call left in it.
+ * Nothing in it needs to start at zero (each pass writes every slot it later reads), but two calls that overlap on
+ * the GPU -- different streams, or different threads, without an ordering between them -- race on it and both
+ * results are garbage.  Calls on one stream are safe back to back.
+ * Summation order: one partial per row, rows combined in index order -- fixed, and independent of the GPU's SM count;
+ * not the order of dnslab_scalar_stats or of a plain loop (agreement ~1e-13 relative). */
+#define DNSLAB_STATIC_MAX_ROWS 65536
+int dnslab_scalar_stats_static(const double *c, const uint8_t *mask, int32_t nx, int32_t ny, int32_t nz,
+                               const int32_t lo[3], const int32_t size[3], void *cuda_stream, double *out);
 
 /* ---- NEXT-4: Lagrangian particles, eqs. 10-13 ------------------------------------------
  * dnslab_particles_attach: from now on every time step of dnslab_step ends with one implicit Euler step of size

@@ -12,7 +12,7 @@ LIB_PATH = os.path.join(_HERE, "libdnslab.so")
 
 SYMBOLS = ["dnslab_workspace_bytes", "dnslab_create", "dnslab_set_fields", "dnslab_step", "dnslab_poisson",
            "dnslab_rfft3", "dnslab_irfft3", "dnslab_fields", "dnslab_get_fields", "dnslab_launch_count", "dnslab_profile", "dnslab_profile_read",
-           "dnslab_courant", "dnslab_set_dt", "dnslab_scalar_stats", "dnslab_particles_attach", "dnslab_destroy", "dnslab_strerror"]
+           "dnslab_courant", "dnslab_set_dt", "dnslab_scalar_stats", "dnslab_scalar_stats_static", "dnslab_particles_attach", "dnslab_destroy", "dnslab_strerror"]
 KERNEL_CLASSES = ["rk_stage", "div", "fft_x", "fft_y", "fft_z_solve", "project", "eq9_sparse", "filter", "reduce", "particles",
                   "fft_xy", "fft_yz_solve"]
 
@@ -63,6 +63,8 @@ def lib():
         L.dnslab_courant.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.dnslab_set_dt.argtypes = [C.c_void_p, C.c_double]
         L.dnslab_scalar_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_double)]
+        L.dnslab_scalar_stats_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int32),
+                                                 C.POINTER(C.c_int32), C.c_void_p, C.c_void_p]
         L.dnslab_particles_attach.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.dnslab_destroy.argtypes = [C.c_void_p]
         L.dnslab_strerror.argtypes = [C.c_int]
@@ -118,6 +120,28 @@ def _addr(x, dtype="float64"):
     if not x.flags["C_CONTIGUOUS"]:
         raise DnslabError("buffer must be contiguous")
     return x.ctypes.data
+
+
+STATIC_MAX_ROWS = 65536  # DNSLAB_STATIC_MAX_ROWS
+
+
+def scalar_stats_static(c, mask, lo, size, out, stream=None):
+    """dnslab_scalar_stats_static: (mean, std, count) of c over the fluid cells of the index box lo, size (x,y,z),
+    for callers that cannot allocate device memory (a monitor handed borrowed pointers while the HBM is fully
+    committed; code that must not stall the device with a cudaMalloc).  Allocates nothing: c (float64 CUDA,
+    (nz, ny, nx)), mask (uint8 CUDA, non-zero = fluid, or None) and out (float64 CUDA, 3 elements) all come from
+    the caller; the scratch is a 1 MiB array inside the library, shared by every call on the device, so calls
+    must not overlap on the GPU.  Asynchronous on `stream` (a torch stream; None = the default stream).  Boxes
+    with size[1]*size[2] > STATIC_MAX_ROWS raise ("... more rows ... than the static scratch array holds")."""
+    nz, ny, nx = (int(s) for s in c.shape)
+    if not (c.is_cuda and out.is_cuda and out.numel() >= 3 and (mask is None or (mask.is_cuda and tuple(mask.shape) == tuple(c.shape)))):
+        raise DnslabError("c, mask and out must be CUDA tensors; mask shaped like c; out with 3 elements")
+    a = (C.c_int32 * 3)(*[int(x) for x in lo])
+    b = (C.c_int32 * 3)(*[int(x) for x in size])
+    _check(lib().dnslab_scalar_stats_static(_addr(c), _addr(mask, "uint8"), nx, ny, nz, a, b,
+                                            stream.cuda_stream if stream is not None else None, _addr(out)),
+           "dnslab_scalar_stats_static")
+    return out
 
 
 class Solver:

@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -745,6 +746,7 @@ const char *dnslab_strerror(int code)
     case DNSLAB_ENOMEM: return "workspace too small";
     case DNSLAB_ECUDA: return "CUDA error";
     case DNSLAB_EARCH: return "no sm_100 device";
+    case DNSLAB_ELIMIT: return "box has more rows (size[1]*size[2]) than the static scratch array holds";
     }
     return "unknown error";
 }
@@ -1209,3 +1211,67 @@ int dnslab_destroy(dnslab_t *h)
 }
 
 } // extern "C"
+
+// ---- dnslab_scalar_stats_static: the one entry point that needs no device memory from anybody ---------------------------
+// Its scratch (one sum and one count per row of the box) lives in this array, which is part of the library's image: every
+// GPU that loads libdnslab.so carries these 1 MiB from the moment the module is loaded until the process exits, used or
+// not.  In HOST code the name g_static_scratch is only a handle for the symbol, not a device address -- handing it to a
+// kernel would fault, or quietly scribble over host memory on systems where the GPU can reach it -- so the host asks
+// the runtime for the address once per device (static_scratch below) and passes that to the kernels.
+static __device__ __align__(256) double g_static_scratch[2 * DNSLAB_STATIC_MAX_ROWS];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+double *g_static_ptr[STATIC_MAX_DEVICES]; // device address of g_static_scratch on each device; null until its first call
+
+// Address of the static scratch array on the CURRENT device; looked up (and the device checked) on the first call
+// made with that device current, remembered afterwards.
+int static_scratch(double **ptr)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return DNSLAB_EARCH;
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return DNSLAB_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (g_static_ptr[dev] == nullptr) {
+        int major = 0;
+        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10) return DNSLAB_EARCH;
+        void *p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_static_scratch) != cudaSuccess || p == nullptr) return DNSLAB_ECUDA;
+        g_static_ptr[dev] = static_cast<double *>(p);
+    }
+    *ptr = g_static_ptr[dev];
+    return DNSLAB_OK;
+}
+} // namespace
+
+extern "C" int dnslab_scalar_stats_static(const double *c, const uint8_t *mask, int32_t nx, int32_t ny, int32_t nz, const int32_t lo[3],
+                                          const int32_t size[3], void *cuda_stream, double *out)
+{
+    if (!c || !lo || !size || !out) return DNSLAB_EINVAL;
+    if (!pow2(nx) || !pow2(ny) || !pow2(nz) || nx < 8 || nx > 2048 || ny < 8 || ny > 1024 || nz < 8 || nz > 1024) return DNSLAB_EINVAL;
+    const int nn[3] = {nx, ny, nz};
+    dnsred::BoxArgs a;
+    a.c = c;
+    a.face = mask;
+    a.nx = nx; a.ny = ny; a.nz = nz;
+    a.count = 1;
+    for (int d = 0; d < 3; ++d) {
+        if (size[d] < 1 || size[d] > nn[d]) return DNSLAB_EINVAL;
+        a.lo[d] = ((lo[d] % nn[d]) + nn[d]) % nn[d];
+        a.size[d] = size[d];
+        a.count *= (size_t)size[d];
+    }
+    const size_t rows = (size_t)size[1] * (size_t)size[2];
+    if (rows > (size_t)DNSLAB_STATIC_MAX_ROWS) return DNSLAB_ELIMIT;
+    double *part = nullptr;
+    if (int rc = static_scratch(&part)) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const unsigned R = (unsigned)rows, G = (R + 7u) / 8u;
+    // nothing in `part` has to start at zero: each pass writes slots 0..R-1 (and R..2R-1) before k_box_final reads exactly those
+    dnsred::k_box_rows<0><<<G, 256, 0, st>>>(a, R, out, part);
+    dnsred::k_box_final<0><<<1, 256, 0, st>>>(part, (int)R, out);
+    dnsred::k_box_rows<1><<<G, 256, 0, st>>>(a, R, out, part);
+    dnsred::k_box_final<1><<<1, 256, 0, st>>>(part, (int)R, out);
+    return cudaPeekAtLastError() == cudaSuccess ? DNSLAB_OK : DNSLAB_ECUDA;
+}

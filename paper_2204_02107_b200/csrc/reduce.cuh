@@ -186,4 +186,69 @@ template <int PASS> __global__ void __launch_bounds__(256) k_box_final(const dou
     }
 }
 
+// Variant of k_box_partial for dnslab_scalar_stats_static (the entry point whose scratch is the library's static
+// device array): ONE partial per row (j, k) of the box instead of one per block -- part[row] holds the row's sum,
+// part[rows + row] its fluid-cell count (PASS 0) -- so the number of scratch slots follows from the box alone and the
+// result does not depend on how many SMs the device has.  One warp per row, lanes stride along x, lane sums folded by
+// a shuffle tree (fixed order).  Every slot k_box_final<PASS>(part, rows, res) reads is written here first, whatever
+// an earlier call left behind.  a.face is the CALLER's mask here: any non-zero byte is a fluid cell (k_box_partial
+// reads the solver's face bytes, bit 0).
+template <int PASS>
+__global__ void __launch_bounds__(256) k_box_rows(const BoxArgs a, unsigned rows, const double *__restrict__ res, double *__restrict__ part)
+{
+    const unsigned row = blockIdx.x * 8u + (threadIdx.x >> 5);
+    if (row >= rows) return; // whole warps leave together
+    const int lane = threadIdx.x & 31;
+    const double mean = PASS == 1 ? res[0] : 0.0;
+    const unsigned k = row / (unsigned)a.size[1], j = row - k * (unsigned)a.size[1];
+    const size_t rowo = (size_t)a.nx * ((size_t)((a.lo[1] + j) & (a.ny - 1)) + (size_t)a.ny * ((a.lo[2] + k) & (a.nz - 1)));
+    const double *cr = a.c + rowo;
+    const uint8_t *fr = a.face != nullptr ? a.face + rowo : nullptr;
+    double s = 0.0, cnt = 0.0;
+    // 16-byte loads where the segment is even, does not wrap and the caller's buffers are aligned for them
+    if (((a.lo[0] | a.size[0]) & 1) == 0 && a.lo[0] + a.size[0] <= a.nx && ((uintptr_t)a.c & 15) == 0 && ((uintptr_t)a.face & 1) == 0) {
+        const double2 *cr2 = reinterpret_cast<const double2 *>(cr + a.lo[0]);
+        const uchar2 *fr2 = fr != nullptr ? reinterpret_cast<const uchar2 *>(fr + a.lo[0]) : nullptr;
+#pragma unroll 4
+        for (int i = lane; i < a.size[0] / 2; i += 32) {
+            const double2 cv = __ldg(cr2 + i);
+            uchar2 f = make_uchar2(1, 1);
+            if (fr2 != nullptr) f = fr2[i];
+            const bool f0 = f.x != 0, f1 = f.y != 0;
+            if (PASS == 0) {
+                s += f0 ? cv.x : 0.0;
+                s += f1 ? cv.y : 0.0;
+                cnt += (f0 ? 1.0 : 0.0) + (f1 ? 1.0 : 0.0);
+            } else {
+                const double d0 = cv.x - mean, d1 = cv.y - mean;
+                s += f0 ? d0 * d0 : 0.0;
+                s += f1 ? d1 * d1 : 0.0;
+            }
+        }
+    } else {
+#pragma unroll 4
+        for (int i = lane; i < a.size[0]; i += 32) {
+            const int x = (a.lo[0] + i) & (a.nx - 1);
+            const bool fluid = fr == nullptr || fr[x] != 0;
+            const double cv = __ldg(cr + x);
+            if (PASS == 0) {
+                s += fluid ? cv : 0.0;
+                cnt += fluid ? 1.0 : 0.0;
+            } else {
+                const double dv = cv - mean;
+                s += fluid ? dv * dv : 0.0;
+            }
+        }
+    }
+#pragma unroll
+    for (int sh = 16; sh > 0; sh >>= 1) {
+        s += __shfl_down_sync(0xffffffffu, s, sh);
+        if (PASS == 0) cnt += __shfl_down_sync(0xffffffffu, cnt, sh);
+    }
+    if (lane == 0) {
+        part[row] = s;
+        if (PASS == 0) part[rows + row] = cnt;
+    }
+}
+
 } // namespace dnsred
