@@ -100,6 +100,8 @@ def ncu_traffic(path, cls, case):
     except ValueError:
         return None, "export lacks dram__bytes_read.sum / dram__bytes_write.sum"
     pat = re.compile(CLASS_KERNELS.get(cls, cls))
+    if units[cr] not in _UNIT or units[cw] not in _UNIT:
+        return None, f"unknown unit {units[cr]!r} / {units[cw]!r} in {os.path.relpath(path, ROOT)}"
     vals = [float(r[cr]) * _UNIT[units[cr]] + float(r[cw]) * _UNIT[units[cw]] for r in data if pat.search(r[cn])]
     if not vals:
         return None, f"no {cls} kernel in {os.path.relpath(path, ROOT)}"
@@ -239,6 +241,14 @@ def cpu_baseline(case, cfg):
                               "sample": f"{where}, 1 step on 1 thread ({sec1:.1f} s/step)"}}
 
 
+def workload_name(config, case):
+    """config.workload: the same string on the GPU arm and on the reference arm (the driver compares them)."""
+    N = int(case["shape"][0]) * int(case["shape"][1]) * int(case["shape"][2])
+    masked = case["mask"] is not None
+    return (f"config {config}: {case['name']} ({N} cells), n_piter={case['n_piter']}, "
+            f"{'masked room with inlet source' if masked else 'periodic box'}")
+
+
 def run_reference(args):
     """--impl reference: the oracle (this tier's reference arm) timed on the host cores, on the bench workload
     itself (config 5: half resolution); every timed step is one oracle step; rank 0 only."""
@@ -257,8 +267,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
         "warmup": warm, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"config {args.config}: {case['name']} ({case['shape'][2]}x{case['shape'][1]}x{case['shape'][0]}), "
-                               f"n_piter={case['n_piter']}; CPU oracle, not a GPU run; steps capped at 5"},
+        "config": {"workload": workload_name(args.config, case), "grid": list(case["shape"][::-1]), "n_piter": case["n_piter"],
+                   "arm": "CPU oracle on the host cores, not a GPU run; steps capped at 5"},
         "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -363,8 +373,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"config {args.config}: {case['name']} ({N} cells), n_piter={P}, "
-                                   f"{'masked room with inlet source' if masked else 'periodic box'}",
+            "config": {"workload": workload_name(args.config, case),
                        "grid": list(case["shape"][::-1]), "n_piter": P, "flags": args.flags,
                        "l2": "working set 19 fields x %.0f MB >> 126 MB L2, no flush needed" % (8 * N / 1e6),
                        "parallelism": "replicas only" if world > 1 else "single GPU"},

@@ -97,8 +97,8 @@ int dnslab_set_fields(dnslab_t *h, const double *u, const double *v, const doubl
 int dnslab_step(dnslab_t *h, int32_t n);
 
 /* One Poisson solve with the beta term off: p = F^-1[F[rhs]/lambda], null modes 0 (eq. 9 with
- * beta = 1).  rhs and p are DEVICE pointers to nx*ny*nz doubles, 16-byte aligned; they may alias.  Does not
- * touch the solver's own pressure. */
+ * beta = 1).  rhs and p are DEVICE pointers to nx*ny*nz doubles, 16-byte aligned (else DNSLAB_EINVAL); they may
+ * alias.  Does not touch the solver's own pressure. */
 int dnslab_poisson(dnslab_t *h, const double *rhs, double *p);
 
 /* The transform of the solve on its own (testing aid: north_star names a real-to-complex transform; the solve itself
@@ -107,7 +107,7 @@ int dnslab_poisson(dnslab_t *h, const double *rhs, double *p);
  *   out[m + (nx/2+1)*(ky + ny*kz)] = sum_{i,j,k} in[i + nx*(j + ny*k)] exp(-2 pi i (m i/nx + ky j/ny + kz k/nz)),
  *   unnormalised, m = 0..nx/2.  Computed with the single-axis passes of the solve (x, y, z) plus one untangling kernel.
  * dnslab_irfft3: the inverse (in = such a half spectrum, Hermitian; out = nx*ny*nz doubles), includes the 1/N.
- * in and out must not overlap.  Both use the solver's work array: do not call between dnslab_step launches on
+ * in and out must be 16-byte aligned and must not overlap (either: DNSLAB_EINVAL).  Both use the solver's work array: do not call between dnslab_step launches on
  * another stream.  PAPER.md:43 ("fft"), eq. 9 PAPER.md:102. */
 int dnslab_rfft3(dnslab_t *h, const double *in, double *out);
 int dnslab_irfft3(dnslab_t *h, const double *in, double *out);

@@ -1036,12 +1036,22 @@ int dnslab_step(dnslab_t *h, int32_t nsteps)
 int dnslab_poisson(dnslab_t *h, const double *rhs, double *p)
 {
     if (!h || !rhs || !p) return DNSLAB_EINVAL;
+    if (((uintptr_t)rhs | (uintptr_t)p) & 15) return DNSLAB_EINVAL; // every pass moves 16-byte pairs
     return poisson_solve(h, rhs, nullptr, p, false);
+}
+
+// true if [a, a + na) and [b, b + nb) share a byte
+static bool ranges_overlap(const void *a, size_t na, const void *b, size_t nb)
+{
+    const uintptr_t a0 = (uintptr_t)a, b0 = (uintptr_t)b;
+    return a0 < b0 + nb && b0 < a0 + na;
 }
 
 int dnslab_rfft3(dnslab_t *h, const double *in, double *out)
 {
     if (!h || !in || !out) return DNSLAB_EINVAL;
+    if (((uintptr_t)in | (uintptr_t)out) & 15) return DNSLAB_EINVAL;
+    if (ranges_overlap(in, h->n * sizeof(double), out, (size_t)(h->P.nx / 2 + 1) * h->P.ny * h->P.nz * sizeof(c2))) return DNSLAB_EINVAL;
     const int M = h->P.nx / 2;
     dnsfft::PoissonRhsArgs ra{};
     c2 *W = reinterpret_cast<c2 *>(h->W);
@@ -1057,6 +1067,8 @@ int dnslab_rfft3(dnslab_t *h, const double *in, double *out)
 int dnslab_irfft3(dnslab_t *h, const double *in, double *out)
 {
     if (!h || !in || !out) return DNSLAB_EINVAL;
+    if (((uintptr_t)in | (uintptr_t)out) & 15) return DNSLAB_EINVAL;
+    if (ranges_overlap(in, (size_t)(h->P.nx / 2 + 1) * h->P.ny * h->P.nz * sizeof(c2), out, h->n * sizeof(double))) return DNSLAB_EINVAL;
     const int M = h->P.nx / 2;
     dnsfft::PoissonRhsArgs ra{};
     c2 *W = reinterpret_cast<c2 *>(h->W);

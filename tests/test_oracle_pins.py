@@ -798,3 +798,171 @@ def test_P17_attached_particles_follow_the_stepped_field():
         b.step(1)
         b.particles_step(st_b, 1.2, (0, 0, -9.81))
     assert np.array_equal(st_a, st_b) and not np.array_equal(st_a[:3], _particles([[1.0, 2.0, 3.0, 0, 0, 0, 1e-3, 1000.0]])[:3])
+
+
+# ---------------------------------------------------------------- pins added in round 3 ("What's weak" 1)
+def _model_step(o, Q, p, dt, P, flags):
+    """SURVEY.md 8(c)'s pseudo-code of one step written out here from the oracle's separately pinned operators
+    (rhs: P5-P9/P18, div and project: P4, poisson_rhs: the eq. 9 fixed-point pin, poisson: P1-P3).  PAPER.md:43 (RK4,
+    projection once per step), PAPER.md:104 (eq. 9 restarts "from the previous available value of pressure": p is
+    state), R29 (flags bit 1: each stage projection iterates on a COPY of p^n and leaves p^n untouched)."""
+    a, b = (0.5, 0.5, 1.0), (1.0 / 6.0, 1.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0)
+    Qc, Qs = [q.copy() for q in Q], [q.copy() for q in Q]
+    for s in range(4):
+        F = o.rhs(*Qs)
+        for m in range(4):
+            Qc[m] = Qc[m] + (b[s] * dt) * F[m]
+            if s < 3:
+                Qs[m] = Q[m] + (a[s] * dt) * F[m]
+        if s < 3 and flags & 2:
+            ps = p.copy()
+            d = o.div(Qs[0], Qs[1], Qs[2])
+            for _ in range(P):
+                ps = o.poisson(o.poisson_rhs(d, ps))
+            Qs[0], Qs[1], Qs[2] = o.project(Qs[0], Qs[1], Qs[2], ps)
+    d = o.div(Qc[0], Qc[1], Qc[2])
+    for _ in range(P):
+        p = o.poisson(o.poisson_rhs(d, p))
+    u, v, w = o.project(Qc[0], Qc[1], Qc[2], p)
+    return [u, v, w, Qc[3]], p
+
+
+@pytest.mark.parametrize("flags", [0, 2])
+def test_P19_step_orchestration_two_steps_warm_started_pressure(flags):
+    """dnsref_step over TWO steps of a masked duct with sources and P = 3 equals the model above: the pressure the
+    first step ends with is where the second step's eq. 9 iterations start (a cold start p = 0 in every step, or stage
+    projections that iterate on p itself instead of a copy, change step 2 / the final p and turn this red)."""
+    case = cases.duct_room(32, 16, 16, steps=2)
+    P = 3
+    kw = dict(nu=case["nu"], alpha_c=case["alpha_c"], dt=case["dt"], mask=case["mask"], sources=case["sources"],
+              body=case["body"], n_piter=P)
+    o = mk(case["shape"], case["d"], flags=flags, **kw)
+    ops = mk(case["shape"], case["d"], **kw)                    # operators only; never stepped
+    o.set_fields(case["u"], case["v"], case["w"], case["c"])
+    ops.set_fields(case["u"], case["v"], case["w"], case["c"])
+    f0 = ops.fields()                                           # masked initial data
+    Q, p = [f0[k] for k in "uvwc"], np.zeros(case["shape"])
+    for step in (1, 2):
+        o.step(1)
+        Q, p = _model_step(ops, Q, p, case["dt"], P, flags)
+        f = o.fields()
+        for k, m in zip("uvwcp", Q + [p]):
+            assert np.abs(f[k] - m).max() <= 1e-15 * max(np.abs(m).max(), 1e-300), (step, k)
+    assert np.abs(p).max() > 0
+    # the model run cold (p = 0 at the start of step 2) is a different answer: the pin can tell the two apart
+    o1 = mk(case["shape"], case["d"], flags=flags, **kw)
+    o1.set_fields(case["u"], case["v"], case["w"], case["c"])
+    o1.step(1)
+    f1 = o1.fields()
+    Qcold, pcold = _model_step(ops, [f1[k] for k in "uvwc"], np.zeros(case["shape"]), case["dt"], P, flags)
+    assert np.abs(pcold - p).max() > 1e-6 * np.abs(p).max()
+
+
+def test_P19_warm_start_leaves_a_smaller_masked_residual_than_a_cold_start():
+    """SURVEY.md 8(c) S14 / PAPER.md:104: with the same number of eq. 9 iterations, a step that starts from the previous
+    pressure ends with a smaller divergence in the fluid than one that starts from zero (the survey's probe found a
+    factor ~10 after 100 steps; after 10 steps of this small duct the factor is already > 1.5)."""
+    case = cases.duct_room(32, 16, 16, steps=10)
+    beta = case["mask"].astype(float)
+    kw = dict(nu=case["nu"], alpha_c=case["alpha_c"], dt=case["dt"], mask=case["mask"], sources=case["sources"],
+              body=case["body"], n_piter=4)
+    o = mk(case["shape"], case["d"], **kw)
+    o.set_fields(case["u"], case["v"], case["w"], case["c"])
+    o.step(9)
+    f9 = o.fields()
+    o.step(1)
+    fw = o.fields()
+    warm = np.abs(o.div(fw["u"], fw["v"], fw["w"]) * beta).max()
+    oc = mk(case["shape"], case["d"], **kw)                                    # same state, pressure forgotten
+    oc.set_fields(f9["u"], f9["v"], f9["w"], f9["c"])
+    oc.step(1)
+    fc = oc.fields()
+    cold = np.abs(oc.div(fc["u"], fc["v"], fc["w"]) * beta).max()
+    assert warm > 0 and cold > 1.5 * warm, (warm, cold)
+
+
+def test_P20_scalar_wall_flux_vanishes_on_every_axis():
+    """eq. 4, dc/dn = 0 at the immersed boundary: in a closed room with walls on all six faces and an
+    obstacle, c = 1 in the fluid (0 in the solid) and no flow, the scalar right-hand side is exactly zero in every
+    cell -- each face towards a solid cell carries no diffusive flux, on the x, y and z faces alike.  A compact second
+    difference on any axis would see the jump from 1 to 0 at that axis' walls."""
+    shape = (12, 10, 16)
+    mask = np.zeros(shape, dtype=np.uint8)
+    mask[2:-2, 2:-2, 2:-2] = 1
+    mask[5:8, 4:6, 6:11] = 0                                                    # an obstacle with faces on all axes
+    o = mk(shape, (0.3, 0.2, 0.25), nu=0.01, alpha_c=0.7, dt=0.1, mask=mask)
+    z = np.zeros(shape)
+    F = o.rhs(z, z, z, mask.astype(float))
+    assert np.all(F[3] == 0.0)
+    # and each axis on its own: a slab of solid normal to that axis only
+    for ax in range(3):
+        m = np.ones(shape, dtype=np.uint8)
+        sl = [slice(None)] * 3
+        sl[ax] = slice(0, 2)
+        m[tuple(sl)] = 0
+        oa = mk(shape, (0.3, 0.2, 0.25), alpha_c=0.7, mask=m)
+        assert np.all(oa.rhs(z, z, z, m.astype(float))[3] == 0.0), ax
+        # whereas a c that varies along the wall-normal axis inside the fluid does diffuse (the term is not switched off)
+        ramp = np.arange(shape[ax], dtype=float).reshape([-1 if a == ax else 1 for a in range(3)]) ** 2 * np.ones(shape) * m
+        assert np.abs(oa.rhs(z, z, z, ramp)[3]).max() > 0.1, ax
+
+
+@pytest.mark.parametrize("wall_axis", ["x", "z"])
+def test_P20_poiseuille_fixed_point_with_the_walls_turned(wall_axis):
+    """P9 with the channel turned: walls normal to x (flow along y) and normal to z (flow along x).  The
+    printed parabola (tests/golden/poiseuille.txt) stays an exact fixed point and c = 1 stays 1 in the fluid, which pins
+    the wall treatment of eqs. 2-4 on the two axes P9 does not reach."""
+    rows = [l.split() for l in open(os.path.join(GOLD, "poiseuille.txt")) if not l.startswith("#")]
+    U = np.array([float(r[1]) for r in rows])
+    b, nu, n, h, wall = 1.0e-3, 0.05, 32, 0.25, 2
+    if wall_axis == "x":
+        shape, d, body, flow = (4, 8, n), (h, 0.3, 0.4), (0.0, b, 0.0), "v"
+        prof = U[None, None, :]
+        solid = (slice(None), slice(None))
+        wsl = lambda s: (slice(None), slice(None), s)
+    else:
+        shape, d, body, flow = (n, 4, 8), (0.3, 0.4, h), (b, 0.0, 0.0), "u"
+        prof = U[:, None, None]
+        wsl = lambda s: (s, slice(None), slice(None))
+    mask = np.ones(shape, dtype=np.uint8)
+    mask[wsl(slice(0, wall))] = 0
+    mask[wsl(slice(n - wall, n))] = 0
+    f0 = np.broadcast_to(prof, shape).copy()
+    zero = np.zeros(shape)
+    o = mk(shape, d, nu=nu, alpha_c=nu, dt=0.2, mask=mask, body=body, n_piter=4)
+    init = dict(u=zero, v=zero, w=zero)
+    init[flow] = f0
+    o.set_fields(init["u"], init["v"], init["w"], mask.astype(float))
+    o.step(5)
+    f = o.fields()
+    assert np.abs(f[flow] - f0).max() < 1e-13 * U.max()
+    for k in "uvw":
+        if k != flow:
+            assert np.abs(f[k]).max() < 1e-15
+    assert np.abs(f["p"]).max() < 1e-15
+    assert np.abs(f["c"] - mask).max() < 1e-14
+
+
+def test_P21_heavy_particle_position_is_the_sum_of_its_new_velocities():
+    """eq. 10 by implicit Euler, reading R27: x_p' = x_p + dt u_p' with the NEW particle velocity.
+    A heavy droplet (dt = tau_p / 100) released at rest in a uniform, slow stream (Re_p ~ 6e-6, so C_d = 1 to 6e-5)
+    has u_n = U (1 - r^n), r = 1 / (1 + dt/tau_p), hence x_n - x_0 = dt U (n - r (1 - r^n) / (1 - r)).  After 50 steps
+    the particle has 39 % of the fluid speed; advancing x with the fluid velocity instead would have moved it 3.7 times
+    as far, with the old particle velocity 4 % less far."""
+    nu, rho_f, rho_p, dp, U = 1.6e-5, 1.2, 1000.0, 1.0e-4, 1.0e-6
+    tau_p = rho_p * dp * dp / (18 * rho_f * nu)
+    dt, n = tau_p / 100, 50
+    shape = (8, 8, 8)
+    o = mk(shape, (0.5, 0.5, 0.5), nu=nu, dt=dt)
+    z = np.zeros(shape)
+    o.set_fields(np.full(shape, U), z, z, z)
+    st = _particles([[0.0, 1.3, 2.1, 0.0, 0.0, 0.0, dp, rho_p]])
+    for _ in range(n):
+        o.particles_step(st, rho_f, (0.0, 0.0, 0.0))
+    r = 1.0 / (1.0 + dt / tau_p)
+    un = U * (1 - r ** n)
+    xn = dt * U * (n - r * (1 - r ** n) / (1 - r))
+    assert 0.38 < un / U < 0.40
+    assert abs(st[3, 0] - un) <= 1e-4 * un
+    assert abs(st[0, 0] - xn) <= 1e-4 * xn, (st[0, 0], xn, dt * U * n)
+    assert st[1, 0] == 1.3 and st[2, 0] == 2.1 and st[4, 0] == 0.0 and st[5, 0] == 0.0

@@ -72,7 +72,9 @@ def test_poisson_matches_oracle(shape):
                                    (512, 256, 128), (32, 512, 128), (64, 512, 128), (128, 512, 128), (256, 512, 128),
                                    (32, 1024, 128), (64, 1024, 128), (128, 1024, 128), (32, 64, 128), (32, 32, 256),
                                    (64, 16, 512), (32, 16, 1024), (128, 256, 512), (256, 256, 256), (64, 256, 1024),
-                                   (128, 128, 1024)])
+                                   (128, 128, 1024),
+                                   # NY0 = 1 with nz < 32: k_fft_xy around the cp.async z pass k_fft_z_solve (no TMA route)
+                                   (16, 64, 128), (8, 16, 512), (16, 32, 256)])
 def test_poisson_two_pass_shapes_match_oracle(shape):
     import torch
     rng = np.random.default_rng(sum(shape) + 1)
@@ -195,8 +197,8 @@ def test_config5_three_rooms_eighth_size_20_steps():
 # Full-size cases (north_star: "all five configs match the CPU oracle"; compare at steps 1 and 100).
 # The measured errors are recorded by the tests themselves in the `record_property` of the junit log and tabulated in
 # DESIGN.md section 3 from the log kept under profiles/.
-def _full_size(case, checkpoints, record_property, what):
-    for cp, got, ref in run_both(case, checkpoints):
+def _full_size(case, checkpoints, record_property, what, flags=0):
+    for cp, got, ref in run_both(case, checkpoints, flags=flags):
         errs = {k: relerr(got[k], ref[k]) for k in "uvwcp"}
         record_property(f"{what} step {cp}", " ".join(f"{k}={e:.2e}" for k, e in errs.items()))
         print(f"[parity] {what} step {cp}: " + " ".join(f"{k}={e:.2e}" for k, e in errs.items()), flush=True)
@@ -231,7 +233,14 @@ def test_config5_full_size_one_step(record_property):
         case, what = cases.config(5), "config 5, 1024x512x256"
     else:
         case, what = cases.three_rooms(1024, 512, 128), f"config 5 z-halved to 1024x512x128 ({avail:.0f} GB host RAM available)"
-    _full_size(case, [1], record_property, what)
+    _full_size(case, [1, 10], record_property, what)   # "steps 1, 100 (oracle cost permitting; else 1, 10)": 1 and 10
+
+
+@pytest.mark.slow
+def test_config4_full_size_one_filtered_step(record_property):
+    """NEXT-1 at the size the bench times it (`--flags 1`): eq. 6 filter on 512x256x128 -- 8 x tiles of k_filter_march,
+    64 planes per block -- one step against the oracle."""
+    _full_size(cases.config(4), [1], record_property, "config 4 with the eq. 6 filter (flags=1), 512x256x128", flags=1)
 
 
 # ------------------------------------------------------------------ variants and edge cases
@@ -251,6 +260,21 @@ def test_per_stage_projection_variant():
     case = cases.duct_room(32, 16, 16)
     for cp, got, ref in run_both(case, [1, 5], flags=2):
         compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"flags=2 step {cp}")
+
+
+def test_per_stage_projection_on_the_marching_kernels(record_property):
+    """NEXT-2 where the bench runs it: grids with nx >= 64 take k_rk_march<STAGE, ELIM=false> (the
+    accumulate-form stage kernel) and project every stage field through the same solve as the step's own projection.
+    Masked duct with sources (steps 1 and 10; with the filter too), an unmasked periodic box without sources (the other
+    instantiations), and config 4's room at half size, 256x128x64, where the stage projections go through the two-pass
+    solve."""
+    for case, cps, flags in [(cases.duct_room(128, 64, 64), [1, 10], 2), (cases.duct_room(128, 64, 64), [1, 5], 3),
+                             (cases.periodic_turbulence(64, steps=5), [1, 5], 2), (cases.config(4, shrink=2), [1], 2)]:
+        for cp, got, ref in run_both(case, cps, flags=flags):
+            errs = " ".join(f"{k}={relerr(got[k], ref[k]):.2e}" for k in "uvwcp")
+            record_property(f"flags={flags} {case['name']} step {cp}", errs)
+            print(f"[parity] flags={flags} {case['name']} step {cp}: {errs}", flush=True)
+            compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"flags={flags} {case['name']} step {cp}")
 
 
 def test_eq6_filter_variant():
@@ -304,6 +328,49 @@ def test_next3_courant_set_dt_and_scalar_stats():
     mo, so, no = o.scalar_stats((0, 0, 0), (64, 64, 64))
     assert ns == no == 64 ** 3 and abs(ms - mo) <= 1e-14 and abs(ss - so) <= 1e-12 * so
     s.close()
+
+
+@pytest.mark.parametrize("shape", [(128, 256, 512), (256, 256, 256)])
+def test_next3_courant_fast_path_at_bench_size(shape):
+    """dnslab_courant where its threads make many trips (config 4's and config 3's grids: 28 and 28 trips of 592 blocks):
+    cells are rated with reciprocal multiplies and only those within 1e-14 of the block's running record are evaluated
+    exactly, so the result must still be the oracle's plain loop bit for bit (R24) wherever the
+    maximum sits -- first cell, last cell, a cell met on a late trip, two near-ties one ulp apart in either order --
+    on a noisy field, on a constant field (every cell ties), and with a NaN in one field (skipped by both)."""
+    nz, ny, nx = shape
+    n = nx * ny * nz
+    d = (0.11, 0.07, 0.05)
+    rng = np.random.default_rng(n + 5)
+    base = [rng.standard_normal(shape) for _ in range(3)]
+    zero = np.zeros(shape)
+    s = binding.Solver(shape, d, 1e-3, 1e-3, 1e-2)
+    o = dnsref.Oracle(shape, d, 1e-3, 1e-3, 1e-2)
+
+    def both(u, v, w):
+        s.set_fields(u, v, w, zero)
+        o.set_fields(u, v, w, zero)
+        a, b = s.courant(), o.courant()
+        assert a == b, (a, b)
+        return a
+
+    co_noise = both(*base)
+    assert co_noise > 0
+    late = n - n // 7 + 3                                           # in the last trips of some block
+    for cells in [(0,), (n - 1,), (late,), (n // 2 + 1, 5), (5, n // 2 + 1)]:
+        f = [b.copy() for b in base]
+        for rank, cell in enumerate(cells):
+            for comp, val in zip(f, (40.0, -35.0, 30.0)):
+                comp.reshape(-1)[cell] = val * (1.0 - rank * 2.3e-16)   # the second planted cell is one ulp smaller
+        co = both(*f)
+        assert co > co_noise
+        expect = (abs(f[0].reshape(-1)[cells[0]]) / d[0] + abs(f[1].reshape(-1)[cells[0]]) / d[1] + abs(f[2].reshape(-1)[cells[0]]) / d[2]) * 1e-2
+        assert co == expect
+    both(np.full(shape, 0.3), np.full(shape, -0.2), np.full(shape, 0.1))
+    f = [b.copy() for b in base]
+    f[1].reshape(-1)[n // 3] = np.nan
+    assert both(*f) > 0
+    s.close()
+    o.close()
 
 
 def test_next4_lagrangian_particles():
@@ -474,4 +541,17 @@ def test_create_rejects_bad_arguments():
     assert L.dnslab_create(C.byref(P), None, None, 0, base, None, C.byref(h)) == 0
     assert L.dnslab_step(h, -1) == -1
     assert L.dnslab_poisson(h, None, None) == -1
+    # pointer contracts of include/dnslab.h: 16-byte alignment (the passes move pairs of doubles); rfft3 / irfft3 in and out apart
+    buf = torch.zeros(8 * 8 * 8 + (5 * 8 * 8) * 2 + 16, dtype=torch.float64, device="cuda")
+    b0 = buf.data_ptr()
+    assert b0 % 16 == 0
+    assert L.dnslab_poisson(h, b0 + 8, b0) == -1 and L.dnslab_poisson(h, b0, b0 + 8) == -1
+    assert L.dnslab_poisson(h, b0, b0) == 0                                                   # aliasing is allowed here
+    spec = b0 + 8 * 512
+    assert L.dnslab_rfft3(h, b0 + 8, spec) == -1 and L.dnslab_rfft3(h, b0, spec + 8) == -1    # misaligned
+    assert L.dnslab_rfft3(h, b0, b0) == -1 and L.dnslab_rfft3(h, b0, spec - 16) == -1         # out starts inside in
+    assert L.dnslab_irfft3(h, spec, spec) == -1 and L.dnslab_irfft3(h, spec, spec - 8 * 512 + 16) == -1
+    assert L.dnslab_irfft3(h, spec + 8, b0) == -1
+    assert L.dnslab_rfft3(h, b0, spec) == 0 and L.dnslab_irfft3(h, spec, b0) == 0             # adjacent, not overlapping
+    torch.cuda.synchronize()
     assert L.dnslab_destroy(h) == 0
