@@ -112,6 +112,18 @@ def ncu_traffic(path, cls, case):
     return sum(vals) / len(vals), f"{os.path.relpath(path, ROOT)}: mean of {len(vals)} launches"
 
 
+def default_traffic_csv(args):
+    """The committed `ncu --set full` export that belongs to this line's workload (profiles/<name>.md names the command
+    and the workload); None if no capture of it is committed -- roofline.traffic is then null."""
+    if args.mode == "reductions":
+        name = "r03c_reductions_raw.csv" if args.config == 4 else None
+    elif args.mode == "particles":
+        name = "r03c_particles_raw.csv" if args.config == 4 else None
+    else:
+        name = {4: "r02e_ncu_full_raw.csv", 3: "r03c_c3_raw.csv", 5: "r03c_c5_raw.csv"}.get(args.config)
+    return os.path.join(ROOT, "profiles", name) if name else None
+
+
 def load_peak():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -340,7 +352,7 @@ def run_ours(args):
     breakdown = {k: {"ms_per_step": v[0] / K, "launches_per_step": v[1] / K, "us_per_launch": v[0] / v[1] * 1e3,
                      "GBps_canonical": cb.get(k, 0.0) * N / (v[0] / v[1] * 1e-3) / 1e9,
                      "GBps_moved": mv.get(k, 0.0) * N / (v[0] / v[1] * 1e-3) / 1e9} for k, v in prof.items()}
-    traffic, traffic_src = ncu_traffic(args.traffic_csv, dom, case)
+    traffic, traffic_src = ncu_traffic(args.traffic_csv or default_traffic_csv(args), dom, case)
     step_bytes = (canonical_bytes_per_cell(P, masked) + (cb["filter"] if args.flags & 1 else 0.0)) * N
     step_gbs = step_bytes / (ms_max / K * 1e-3) / 1e9
     moved_step = sum(mv.get(k, 0.0) * v[1] / K for k, v in prof.items())   # bytes per cell per step actually required
@@ -437,6 +449,8 @@ def run_extra(args):
     t0 = time.time()
     base = {"n_gpus": 1, "steps": K, "warmup": W, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic"}
+    traffic, traffic_src = ncu_traffic(args.traffic_csv or default_traffic_csv(args),
+                                       "k_courant" if args.mode == "reductions" else "particles", case)
     if args.mode == "reductions":
         # dnslab_courant: one streaming read of u, v, w (24 B/cell); dnslab_scalar_stats over the whole box: two
         # passes over c and the mask byte (2 x 9 B/cell).  Both calls synchronise; the device time is taken from the
@@ -462,7 +476,7 @@ def run_extra(args):
                                        f"dnslab_scalar_stats over the whole box, {K} calls each"},
                    gpu_launches=launches,
                    roofline={"bound": "hbm", "kernel": "reduce (k_courant)", "achieved": co_gbs, "peak": peak, "unit": "GB/s",
-                             "frac": co_gbs / peak, "traffic": None, "peak_source": peak_src},
+                             "frac": co_gbs / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src},
                    scalar_stats={"ms_per_call": ms_st / K, "GBps": st_gbs, "frac": st_gbs / peak,
                                  "bytes_per_cell": 2 * 8.0 + (2.0 if masked else 0.0), "launches_timed_per_call": n_st / K})
     else:
@@ -495,7 +509,7 @@ def run_extra(args):
                            "particles": n},
                    gpu_launches=launches,
                    roofline={"bound": "hbm", "kernel": "particles (k_particles)", "achieved": gbs, "peak": peak, "unit": "GB/s",
-                             "frac": gbs / peak, "traffic": None, "peak_source": peak_src,
+                             "frac": gbs / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                              "note": "304 B per particle (8 state reads, 6 writes, 24 gathered velocities)"},
                    share_of_step=ms_p / tot, fluid_step_ms=(tot - ms_p) / K)
     s.synchronize()
@@ -519,7 +533,7 @@ def main():
     ap.add_argument("--mode", default="step", choices=["step", "reductions", "particles"],
                     help="step: the headline line; reductions / particles: the NEXT-3 / NEXT-4 lines")
     ap.add_argument("--particles", type=int, default=1000000, help="--mode particles: how many")
-    ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r02e_ncu_full_raw.csv"),
+    ap.add_argument("--traffic-csv", default=None,
                     help="ncu --page raw --csv export of a --set full capture of this workload (roofline.traffic)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")

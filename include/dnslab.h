@@ -121,6 +121,10 @@ int dnslab_fields(dnslab_t *h, const double **u, const double **v, const double 
  * stream for device and pinned-host destinations; synchronise the stream before reading. */
 int dnslab_get_fields(dnslab_t *h, double *u, double *v, double *w, double *c, double *p);
 
+/* ---- Measurement aids: NOT part of the method ---------------------------------------------------------------
+ * dnslab_launch_count, dnslab_profile, dnslab_profile_read and the DNSLAB_K_* classes exist for bench.py and the
+ * tests (launch accounting, per-kernel device times).  Nothing the paper defines depends on them; a user of the
+ * solver never needs to call them, and the class list follows this implementation's kernels, not the paper. */
 /* Number of kernels the library has launched on this handle since create (for bench accounting). */
 int64_t dnslab_launch_count(const dnslab_t *h);
 

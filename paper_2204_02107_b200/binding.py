@@ -41,36 +41,42 @@ def lib():
     """Load libdnslab.so (built in-tree by paper_2204_02107_b200/build.py).  Fails loudly."""
     global _lib
     if _lib is None:
-        if not os.path.exists(LIB_PATH):
-            raise DnslabError(f"{LIB_PATH} not built: run `python -m paper_2204_02107_b200.build` "
-                              "(there is no CPU fallback)")
-        L = C.CDLL(LIB_PATH)
-        L.dnslab_workspace_bytes.argtypes = [C.POINTER(Params)]
-        L.dnslab_workspace_bytes.restype = C.c_size_t
-        L.dnslab_create.argtypes = [C.POINTER(Params), C.c_void_p, C.POINTER(Source), C.c_int32, C.c_void_p,
-                                    C.c_void_p, C.POINTER(C.c_void_p)]
-        L.dnslab_set_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 5
-        L.dnslab_step.argtypes = [C.c_void_p, C.c_int32]
-        L.dnslab_poisson.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
-        L.dnslab_rfft3.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
-        L.dnslab_irfft3.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
-        L.dnslab_fields.argtypes = [C.c_void_p] + [C.POINTER(C.c_void_p)] * 5
-        L.dnslab_get_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 5
-        L.dnslab_launch_count.argtypes = [C.c_void_p]
-        L.dnslab_launch_count.restype = C.c_int64
-        L.dnslab_profile.argtypes = [C.c_void_p, C.c_int]
-        L.dnslab_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
-        L.dnslab_courant.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
-        L.dnslab_set_dt.argtypes = [C.c_void_p, C.c_double]
-        L.dnslab_scalar_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_double)]
-        L.dnslab_scalar_stats_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int32),
-                                                 C.POINTER(C.c_int32), C.c_void_p, C.c_void_p]
-        L.dnslab_particles_attach.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_double, C.POINTER(C.c_double)]
-        L.dnslab_destroy.argtypes = [C.c_void_p]
-        L.dnslab_strerror.argtypes = [C.c_int]
-        L.dnslab_strerror.restype = C.c_char_p
-        _lib = L
+        _lib = load(LIB_PATH)
     return _lib
+
+
+def load(path):
+    """A library at `path` with the C ABI of include/dnslab.h, argument types declared (lib() loads the product;
+    the GPU tests also load the test-only no-TMA build through this)."""
+    if not os.path.exists(path):
+        raise DnslabError(f"{path} not built: run `python -m paper_2204_02107_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    L.dnslab_workspace_bytes.argtypes = [C.POINTER(Params)]
+    L.dnslab_workspace_bytes.restype = C.c_size_t
+    L.dnslab_create.argtypes = [C.POINTER(Params), C.c_void_p, C.POINTER(Source), C.c_int32, C.c_void_p,
+                                C.c_void_p, C.POINTER(C.c_void_p)]
+    L.dnslab_set_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 5
+    L.dnslab_step.argtypes = [C.c_void_p, C.c_int32]
+    L.dnslab_poisson.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.dnslab_rfft3.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.dnslab_irfft3.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.dnslab_fields.argtypes = [C.c_void_p] + [C.POINTER(C.c_void_p)] * 5
+    L.dnslab_get_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 5
+    L.dnslab_launch_count.argtypes = [C.c_void_p]
+    L.dnslab_launch_count.restype = C.c_int64
+    L.dnslab_profile.argtypes = [C.c_void_p, C.c_int]
+    L.dnslab_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+    L.dnslab_courant.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+    L.dnslab_set_dt.argtypes = [C.c_void_p, C.c_double]
+    L.dnslab_scalar_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_double)]
+    L.dnslab_scalar_stats_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int32),
+                                             C.POINTER(C.c_int32), C.c_void_p, C.c_void_p]
+    L.dnslab_particles_attach.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_double, C.POINTER(C.c_double)]
+    L.dnslab_destroy.argtypes = [C.c_void_p]
+    L.dnslab_strerror.argtypes = [C.c_int]
+    L.dnslab_strerror.restype = C.c_char_p
+    return L
 
 
 def _check(rc, what):

@@ -426,7 +426,11 @@ template <int L> int launch_fft_z_solve_tma(dnslab *h, c2 *data, bool *done)
 
 template <int L> int launch_fft_z_solve_L(dnslab *h, c2 *data)
 {
-    if constexpr (L >= 32) {
+    // The TMA route runs one block per SM with XT <= 16 columns per tile: at nz = 32 and 64 its tiles are only 512 and 1024
+    // points and it loses to the cp.async kernel, which fills every SM (measured, 30 solves each, us per z pass, TMA / cp.async:
+    // 2048x1024x32 476 / 200; 2048x1024x64 612 / 415; 1024x512x64 163 / 110; 2048x512x128 476 / 502; 1024x1024x128 477 / 490;
+    // 1024x512x256 429 / 605; no difference on small grids).  So: TMA from nz = 128 up.
+    if constexpr (L >= 128) {
         bool done = false;
         const int rc = launch_fft_z_solve_tma<L>(h, data, &done);
         if (rc || (done && !h->prepare)) return rc;
@@ -819,6 +823,7 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
     h->wmap_ok = false;
     h->wmapz_ok = false;
     h->tma_encode = nullptr;
+#ifndef DNSLAB_TEST_NO_TMA // test-only build (libdnslab_notma.so): the encoder stays null, so every fallback below is the path taken
     {
         void *fp = nullptr;
         cudaDriverEntryPointQueryResult qres;
@@ -827,6 +832,7 @@ int dnslab_create(const dnslab_params_t *params, const uint8_t *mask, const dnsl
             h->tma_encode = fp;
         (void)cudaGetLastError();
     }
+#endif
     if (h->rk_kc > 0) {
         const cuuint64_t gdim[3] = {(cuuint64_t)params->nx, (cuuint64_t)params->ny, (cuuint64_t)params->nz};
         const cuuint32_t box[3] = {(cuuint32_t)dnsst::RKM_SW, (cuuint32_t)dnsst::RKM_ROWS, 1u};

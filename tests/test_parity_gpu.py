@@ -93,6 +93,40 @@ def test_poisson_two_pass_shapes_match_oracle(shape):
     assert torch.equal(buf, p)
 
 
+@pytest.fixture
+def notma_library():
+    """The test-only build of the same sources with -DDNSLAB_TEST_NO_TMA (paper_2204_02107_b200/build.py): dnslab_create
+    never obtains cuTensorMapEncodeTiled there, so every route that needs a tensor map falls back -- as it would on a driver
+    without that entry point."""
+    from paper_2204_02107_b200 import build
+    saved = binding._lib
+    binding._lib = binding.load(build.build_notma())
+    yield
+    binding._lib = saved
+
+
+def test_fallback_paths_without_tensor_maps(notma_library):
+    """Without tensor maps: the two-pass solve with a split of y is off (five single-axis passes), the z pass is the
+    cp.async kernel k_fft_z_solve also for nz >= 128, and k_rk_march copies every plane tile with cp.async.  Solves and
+    stepped cases against the oracle at the usual tolerances."""
+    import torch
+    d = (0.11, 0.07, 0.05)
+    for shape, launches in [((64, 256, 128), 5), ((128, 128, 256), 5), ((32, 64, 128), 3), ((256, 16, 512), 3), ((64, 32, 2048), 5)]:
+        rhs = np.random.default_rng(sum(shape) + 11).standard_normal(shape)
+        s = binding.Solver(shape, d, 0.1, 0.1, 0.1)
+        n0 = s.launch_count()
+        p = s.poisson(torch.from_numpy(rhs).cuda())
+        assert s.launch_count() - n0 == launches, shape
+        s.synchronize()
+        o = dnsref.Oracle(shape, d, 0.1, 0.1, 0.1)
+        assert relerr(p.cpu().numpy(), o.poisson(rhs)) <= 1e-13 * np.log2(max(shape)), shape
+        s.close()
+        o.close()
+    for case, cps in [(cases.duct_room(128, 64, 64), [1, 5]), (cases.config(4, shrink=2), [1, 3]), (cases.periodic_turbulence(64, steps=3), [1, 3])]:
+        for cp, got, ref in run_both(case, cps):
+            compare(got, ref, TOL1 if cp == 1 else TOL100, mask=case["mask"], what=f"no TMA {case['name']} step {cp}")
+
+
 @pytest.mark.parametrize("shape", [(128, 256, 512), (256, 64, 128), (512, 16, 64)])
 def test_poisson_persistent_passes_are_repeatable(shape):
     """The middle pass (k_fft_yz_solve) is a persistent kernel whose two thread groups share a landing buffer and hand
