@@ -72,3 +72,56 @@ def test_product_path_never_touches_the_oracle():
     for f in ("dnsref.c", "dnsref.py"):
         txt = open(os.path.join(ROOT, "oracle", f)).read()
         assert "libdnslab" not in txt and "binding" not in txt and "csrc/" not in txt.replace("paper_2204_02107_b200/csrc/", "")
+
+
+def test_scalar_stats_static_validates_before_touching_the_device(L):
+    """The entry point that allocates nothing checks its arguments -- and the row limit of its static scratch array --
+    before any CUDA call, so the refusals can be seen without a GPU; the pointers below are never dereferenced."""
+    fake = 0x1000
+    lo, size = (C.c_int32 * 3)(0, 0, 0), (C.c_int32 * 3)(8, 8, 8)
+    f = L.dnslab_scalar_stats_static
+    assert f(None, None, 8, 8, 8, lo, size, None, fake) == -1                     # no c
+    assert f(fake, None, 8, 8, 8, lo, size, None, None) == -1                     # no out
+    assert f(fake, None, 8, 12, 8, lo, size, None, fake) == -1                    # ny not a power of two
+    assert f(fake, None, 4096, 8, 8, lo, size, None, fake) == -1                  # nx beyond the library's grids
+    assert f(fake, None, 8, 8, 8, lo, (C.c_int32 * 3)(9, 1, 1), None, fake) == -1  # box wider than the grid
+    assert f(fake, None, 8, 8, 8, lo, (C.c_int32 * 3)(1, 0, 1), None, fake) == -1
+    big = (C.c_int32 * 3)(8, 512, 256)                                            # 131 072 rows > DNSLAB_STATIC_MAX_ROWS
+    assert binding.STATIC_MAX_ROWS == 65536
+    assert f(fake, None, 8, 512, 256, lo, big, None, fake) == -5
+    assert b"static scratch" in L.dnslab_strerror(-5)
+    import torch
+    if not torch.cuda.is_available():
+        ok = (C.c_int32 * 3)(8, 256, 256)                                         # exactly the limit: passes the checks, then no device
+        assert f(fake, None, 8, 256, 256, lo, ok, None, fake) == -4
+
+
+def test_bench_traffic_lookup_and_workload_string():
+    """bench.py host logic: roofline.traffic comes from the committed ncu export of the line's own workload, is None
+    (not an exception) for an export with an unknown unit or of another workload, and both arms name the workload alike."""
+    import argparse
+    import sys
+    import tempfile
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2204_02107_b200 import cases
+    a = argparse.Namespace(config=4, mode="step", traffic_csv=None)
+    t, src = bench.ncu_traffic(bench.default_traffic_csv(a), "rk_stage", {"name": "room512x256x128"})
+    assert t is not None and 1.5e9 < t < 1.7e9, (t, src)                          # 96 B/cell x 16.8 M cells
+    assert bench.ncu_traffic(bench.default_traffic_csv(a), "rk_stage", {"name": "duct128x64x64"})[0] is None
+    assert bench.default_traffic_csv(argparse.Namespace(config=2, mode="step", traffic_csv=None)) is None
+    for cfg, mode, cls, name in [(3, "step", "rk_stage", "turb256"), (5, "step", "rk_stage", "rooms1024x512x256"),
+                                 (4, "reductions", "k_courant", "room512x256x128"), (4, "particles", "particles", "room512x256x128")]:
+        a = argparse.Namespace(config=cfg, mode=mode, traffic_csv=None)
+        assert bench.ncu_traffic(bench.default_traffic_csv(a), cls, {"name": name})[0] is not None, (cfg, mode)
+    with tempfile.TemporaryDirectory() as d:
+        p = os.path.join(d, "x.csv")
+        with open(p, "w") as fh:
+            fh.write('"Kernel Name","dram__bytes_read.sum","dram__bytes_write.sum"\n"","Pbyte","Pbyte"\n"k_rk_march<1>","1","1"\n')
+        with open(os.path.join(d, "x.md"), "w") as fh:
+            fh.write("room512x256x128")
+        t, src = bench.ncu_traffic(p, "rk_stage", {"name": "room512x256x128"})
+        assert t is None and "unknown unit" in src
+    case = cases.config(2)
+    w = bench.workload_name(2, case)
+    assert w.startswith("config 2: duct128x64x64 (524288 cells), n_piter=4")
